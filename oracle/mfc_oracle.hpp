@@ -1,0 +1,381 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// Plain, slow, CPU implementation of the finite-volume right-hand side of the
+// 5-equation (Allaire) multi-component model with stiffened-gas EOS, WENO5-JS +
+// HLLC, SSP-RK3, written step by step from /root/reference/PAPER.md (MFC 5.0,
+// arxiv 2503.07953).  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may use it.  It shares no code with the
+// CUDA path under paper_2503_07953_b200/csrc and neither includes the other.
+//
+// Passages followed (PAPER.md line : section/equation):
+//   57-61   §2.1.1 five-equation model            76  eq.(4) mixture rules
+//   117     §2.2   stiffened-gas EOS              133-143 eqs.(9),(10), div u
+//   151-165 §3.2.1 reconstruction of primitives   187-199 §3.2.2 HLLC
+//   203     §3.3   ghost ("buffer") cells         207-211 §3.4 SSP-RK3
+//   653-654, 664, 668 (§4.2.5) wave-speed, S_M and rho* formulas
+// Readings of silent/garbled points carry the A-numbers of DESIGN.md §3.
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): prim round trip and pure-fluid
+// closed form (O2); WENO linear/closed-form/ENO/mirror/order-5 (O3); HLLC
+// consistency, upwinding, stationary contact, mirror (O4); Sod and water/air
+// exact Riemann solutions, uniform-state, conservation, interface equilibrium,
+// alpha==1 (O2-O6).  cfl_dt (A9) and the clamp (A10) are defined by
+// BASELINE.json only, not by the paper: "parity unpinned" beyond their
+// closed-form definition tests.
+//
+// Everything is a template on the scalar T so that the same text gives the
+// fp64 oracle, a long double adjudicator and an operation-counting build.
+#pragma once
+#include <algorithm>
+#include <cmath>
+#include <cstddef>
+#include <vector>
+
+namespace mfc_oracle {
+
+constexpr int kMaxFluids = 4;
+constexpr int kMaxEq = 2 * kMaxFluids + 3 + 1;
+
+enum { BC_PERIODIC = 0, BC_EXTRAP = 1 };
+enum { RECON_PIECEWISE_CONSTANT = 1, RECON_WENO5_JS = 5 };
+
+// generic helpers so that T may be double, long double or the counting type
+template <class T> inline T o_sqrt(const T& x) { using std::sqrt; return sqrt(x); }
+template <class T> inline T o_abs(const T& x) { return x < T(0) ? T(0) - x : x; }
+template <class T> inline T o_min(const T& a, const T& b) { return b < a ? b : a; }
+template <class T> inline T o_max(const T& a, const T& b) { return a < b ? b : a; }
+// a rational constant a/b of the scheme, formed in T (so that long double gets it to full precision)
+template <class T> inline T o_ratio(int a, int b) { return T(a) / T(b); }
+
+template <class T>
+struct Params {
+  int ndim = 1;            // D, 1..3
+  int n[3] = {1, 1, 1};    // cells; n[d] = 1 for d >= D
+  T dx[3] = {T(1), T(1), T(1)};
+  int nfluids = 1;         // N
+  T gamma[kMaxFluids];     // gamma_i
+  T pi_inf[kMaxFluids];    // pi_inf_i
+  int bc_lo[3] = {0, 0, 0}, bc_hi[3] = {0, 0, 0};
+  T weno_eps = T(1e-16);   // A4
+  T alpha_floor = T(1e-6); // A10
+  int clamp = 0;           // A10
+  int recon = RECON_WENO5_JS;
+
+  int neq() const { return 2 * nfluids + ndim + 1; }  // PAPER.md:704 "two advected species (8 PDEs)" in 3D
+  std::size_t cells() const { return std::size_t(n[0]) * n[1] * n[2]; }
+  // variable slots, identical for q and w (PAPER.md:165 lists them in this order)
+  int i_arho(int i) const { return i; }
+  int i_mom(int d) const { return nfluids + d; }
+  int i_E() const { return nfluids + ndim; }
+  int i_alpha(int i) const { return nfluids + ndim + 1 + i; }
+  // G_i = 1/(gamma_i-1), P_i = gamma_i pi_inf_i/(gamma_i-1)   (from PAPER.md:117 with eq.(4)),
+  // formed once by derive() after gamma/pi_inf are set.
+  T Gc[kMaxFluids], Pc[kMaxFluids];
+  void derive() {
+    for (int i = 0; i < nfluids; ++i) {
+      Gc[i] = T(1) / (gamma[i] - T(1));
+      Pc[i] = (gamma[i] * pi_inf[i]) / (gamma[i] - T(1));
+    }
+  }
+  const T& G(int i) const { return Gc[i]; }
+  const T& P(int i) const { return Pc[i]; }
+};
+
+// O1: ghost cell g in [-3, n+2] -> interior cell supplying its value.
+inline int ghost_index(int g, int n, int bc_lo, int bc_hi) {
+  if (g < 0) return bc_lo == BC_PERIODIC ? ((g % n) + n) % n : 0;
+  if (g >= n) return bc_hi == BC_PERIODIC ? g % n : n - 1;
+  return g;
+}
+
+// O2 (eq.(4), 117, 165): conservative cell -> primitive cell.
+// rho e = Gamma p + Pi with Gamma = sum alpha_i G_i, Pi = sum alpha_i P_i; E = rho e + ke.
+// Returns 0, or 1 if rho <= 0 / not finite (A19).
+template <class T>
+int prim_from_cons_cell(const Params<T>& P, const T* q, T* w) {
+  const int N = P.nfluids, D = P.ndim;
+  T rho = T(0);
+  for (int i = 0; i < N; ++i) rho = rho + q[P.i_arho(i)];
+  T usq = T(0);
+  for (int d = 0; d < D; ++d) {
+    T u = q[P.i_mom(d)] / rho;
+    w[P.i_mom(d)] = u;
+    usq = usq + u * u;
+  }
+  T Gam = T(0), Pi = T(0);
+  for (int i = 0; i < N; ++i) {
+    Gam = Gam + q[P.i_alpha(i)] * P.G(i);
+    Pi = Pi + q[P.i_alpha(i)] * P.P(i);
+  }
+  T ke = (T(0.5) * rho) * usq;
+  w[P.i_E()] = ((q[P.i_E()] - Pi) - ke) / Gam;
+  for (int i = 0; i < N; ++i) {
+    w[P.i_arho(i)] = q[P.i_arho(i)];
+    w[P.i_alpha(i)] = q[P.i_alpha(i)];
+  }
+  return (rho > T(0)) ? 0 : 1;
+}
+
+// mixture sound speed squared at frozen alpha (A5): c^2 = ((Gamma+1) p + Pi)/(Gamma rho);
+// reduces to eq.(6) gamma (p+pi_inf)/rho for a pure fluid.
+template <class T>
+T sound_speed_sq(const T& Gam, const T& Pi, const T& p, const T& rho) {
+  return ((Gam + T(1)) * p + Pi) / (Gam * rho);
+}
+
+// O3 (Jiang-Shu coefficients of the paper's refs [30],[70], A3).
+// Stencil (a,b,c,d,e) = w_{i-2..i+2}.  *left = left-biased value at i+1/2 (q^L of
+// face i+1/2), *right = right-biased value at i-1/2 (q^R of face i-1/2).
+template <class T>
+void weno5_js(const T& a, const T& b, const T& c, const T& d, const T& e, const T& eps, T* left, T* right) {
+  const T c1312 = o_ratio<T>(13, 12), c14 = o_ratio<T>(1, 4);
+  T t0 = a - T(2) * b + c, t1 = b - T(2) * c + d, t2 = c - T(2) * d + e;
+  T s0 = a - T(4) * b + T(3) * c, s1 = b - d, s2 = T(3) * c - T(4) * d + e;
+  T b0 = c1312 * (t0 * t0) + c14 * (s0 * s0);
+  T b1 = c1312 * (t1 * t1) + c14 * (s1 * s1);
+  T b2 = c1312 * (t2 * t2) + c14 * (s2 * s2);
+  // left-biased, ideal weights (1/10, 6/10, 3/10)
+  {
+    T p0 = (T(2) * a - T(7) * b + T(11) * c) / T(6);
+    T p1 = (T(5) * c - b + T(2) * d) / T(6);
+    T p2 = (T(2) * c + T(5) * d - e) / T(6);
+    T a0 = o_ratio<T>(1, 10) / ((b0 + eps) * (b0 + eps));
+    T a1 = o_ratio<T>(6, 10) / ((b1 + eps) * (b1 + eps));
+    T a2 = o_ratio<T>(3, 10) / ((b2 + eps) * (b2 + eps));
+    T s = a0 + a1 + a2;
+    *left = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+  }
+  // right-biased (mirror image), ideal weights (3/10, 6/10, 1/10), same beta
+  {
+    T p0 = (T(5) * b - a + T(2) * c) / T(6);
+    T p1 = (T(2) * b + T(5) * c - d) / T(6);
+    T p2 = (T(11) * c - T(7) * d + T(2) * e) / T(6);
+    T a0 = o_ratio<T>(3, 10) / ((b0 + eps) * (b0 + eps));
+    T a1 = o_ratio<T>(6, 10) / ((b1 + eps) * (b1 + eps));
+    T a2 = o_ratio<T>(1, 10) / ((b2 + eps) * (b2 + eps));
+    T s = a0 + a1 + a2;
+    *right = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+  }
+}
+
+// O4 (S_L,S_R 653-654; S* 664; rho* 668; A5-A8): HLLC at one face with
+// normal direction dir, from reconstructed primitives wL, wR.  Writes F[neq] and the face
+// velocity u_f.  Returns 0, or 1 if a face state is non-physical (A19).
+template <class T>
+int hllc_face(const Params<T>& P, int dir, const T* wL, const T* wR, T* F, T* uf) {
+  const int N = P.nfluids, D = P.ndim, neq = P.neq();
+  const T* w[2] = {wL, wR};
+  T rho[2], Gam[2], Pi[2], E[2], c[2], un[2], p[2];
+  int bad = 0;
+  for (int K = 0; K < 2; ++K) {
+    rho[K] = T(0); Gam[K] = T(0); Pi[K] = T(0);
+    for (int i = 0; i < N; ++i) rho[K] = rho[K] + w[K][P.i_arho(i)];
+    for (int i = 0; i < N; ++i) {
+      Gam[K] = Gam[K] + w[K][P.i_alpha(i)] * P.G(i);
+      Pi[K] = Pi[K] + w[K][P.i_alpha(i)] * P.P(i);
+    }
+    T usq = T(0);
+    for (int d = 0; d < D; ++d) usq = usq + w[K][P.i_mom(d)] * w[K][P.i_mom(d)];
+    p[K] = w[K][P.i_E()];
+    un[K] = w[K][P.i_mom(dir)];
+    E[K] = Gam[K] * p[K] + Pi[K] + (T(0.5) * rho[K]) * usq;
+    T c2 = sound_speed_sq(Gam[K], Pi[K], p[K], rho[K]);
+    if (!(rho[K] > T(0)) || !(c2 > T(0))) bad = 1;
+    c[K] = o_sqrt(c2);
+  }
+  const T SL = o_min(un[0] - c[0], un[1] - c[1]);
+  const T SR = o_max(un[0] + c[0], un[1] + c[1]);
+  const T Sstar = (p[1] - p[0] + rho[0] * un[0] * (SL - un[0]) - rho[1] * un[1] * (SR - un[1])) /
+                  (rho[0] * (SL - un[0]) - rho[1] * (SR - un[1]));
+  // physical flux and conservative state of side K, then the star correction S_K (q*_K - q_K)
+  auto side_flux = [&](int K, bool star, const T& SK) {
+    const T chi = star ? (SK - un[K]) / (SK - Sstar) : T(1);
+    for (int v = 0; v < neq; ++v) F[v] = T(0);
+    for (int i = 0; i < N; ++i) {
+      T qv = w[K][P.i_arho(i)];
+      F[P.i_arho(i)] = qv * un[K];
+      if (star) F[P.i_arho(i)] = F[P.i_arho(i)] + SK * (chi * qv - qv);
+      T av = w[K][P.i_alpha(i)];
+      F[P.i_alpha(i)] = av * un[K];
+      if (star) F[P.i_alpha(i)] = F[P.i_alpha(i)] + SK * (chi * av - av);  // A7
+    }
+    for (int d = 0; d < D; ++d) {
+      T qv = rho[K] * w[K][P.i_mom(d)];
+      F[P.i_mom(d)] = qv * un[K] + (d == dir ? p[K] : T(0));
+      if (star) {
+        T qs = (d == dir) ? chi * rho[K] * Sstar : chi * qv;
+        F[P.i_mom(d)] = F[P.i_mom(d)] + SK * (qs - qv);
+      }
+    }
+    F[P.i_E()] = (E[K] + p[K]) * un[K];
+    if (star) {
+      T Es = chi * (E[K] + (Sstar - un[K]) * (rho[K] * Sstar + p[K] / (SK - un[K])));
+      F[P.i_E()] = F[P.i_E()] + SK * (Es - E[K]);
+    }
+    *uf = star ? un[K] + SK * (chi - T(1)) : un[K];  // HLLC flux of a unit scalar (A7)
+  };
+  // first match in the printed order (A8)
+  if (SL >= T(0)) side_flux(0, false, SL);
+  else if (Sstar >= T(0)) side_flux(0, true, SL);
+  else if (SR > T(0)) side_flux(1, true, SR);
+  else side_flux(1, false, SR);
+  return bad;
+}
+
+// A10: positivity / volume-fraction clamp applied to one cell after each RK stage.
+template <class T>
+void clamp_cell(const Params<T>& P, T* q) {
+  const int N = P.nfluids;
+  for (int i = 0; i < N; ++i) q[P.i_arho(i)] = o_max(q[P.i_arho(i)], T(0));
+  bool marked = false;
+  for (int i = 0; i < N; ++i)
+    if (q[P.i_alpha(i)] < P.alpha_floor) { q[P.i_alpha(i)] = P.alpha_floor; marked = true; }
+  if (marked) {
+    T s = T(0);
+    for (int i = 0; i < N; ++i) s = s + q[P.i_alpha(i)];
+    for (int i = 0; i < N; ++i) q[P.i_alpha(i)] = q[P.i_alpha(i)] / s;
+  }
+}
+
+template <class T>
+struct Solver {
+  Params<T> P;
+  explicit Solver(const Params<T>& p) : P(p) { P.derive(); }
+
+  std::size_t idx(int v, int i, int j, int k) const {
+    return ((std::size_t(v) * P.n[2] + k) * P.n[1] + j) * P.n[0] + i;
+  }
+
+  // mfc_prim_from_cons over the whole grid. Returns the number of cells flagged (A19).
+  long prim_from_cons(const T* q, T* w) const {
+    const int neq = P.neq();
+    const std::size_t nc = P.cells();
+    long bad = 0;
+#pragma omp parallel for reduction(+ : bad) schedule(static)
+    for (long c = 0; c < (long)nc; ++c) {
+      T qc[kMaxEq], wc[kMaxEq];
+      for (int v = 0; v < neq; ++v) qc[v] = q[std::size_t(v) * nc + c];
+      bad += prim_from_cons_cell(P, qc, wc);
+      for (int v = 0; v < neq; ++v) w[std::size_t(v) * nc + c] = wc[v];
+    }
+    return bad;
+  }
+
+  // O5: rhs = L(q).  dir_mask selects directions (bit d), default all.
+  long rhs(const T* q, T* rhs_out, int dir_mask = 7) const {
+    const int neq = P.neq(), N = P.nfluids;
+    const std::size_t nc = P.cells();
+    for (std::size_t t = 0; t < nc * neq; ++t) rhs_out[t] = T(0);
+    long bad = 0;
+    for (int dir = 0; dir < P.ndim; ++dir) {
+      if (!((dir_mask >> dir) & 1)) continue;
+      const int n = P.n[dir];
+      const int d1 = (dir + 1) % 3, d2 = (dir + 2) % 3;  // the two transverse index directions
+      const long nlines = long(P.n[d1]) * P.n[d2];
+#pragma omp parallel for reduction(+ : bad) schedule(static)
+      for (long line = 0; line < nlines; ++line) {
+        int ijk[3];
+        ijk[d1] = int(line % P.n[d1]);
+        ijk[d2] = int(line / P.n[d1]);
+        // primitives along the line with 3 ghost cells each side: wl[(g+3)*neq + v], g = -3..n+2
+        std::vector<T> wl(std::size_t(n + 6) * neq), WL(std::size_t(n + 2) * neq), WR(std::size_t(n + 2) * neq);
+        std::vector<T> Ff(std::size_t(n + 1) * neq), uf(n + 1);
+        for (int g = -3; g < n + 3; ++g) {
+          ijk[dir] = ghost_index(g, n, P.bc_lo[dir], P.bc_hi[dir]);
+          T qc[kMaxEq];
+          for (int v = 0; v < neq; ++v) qc[v] = q[idx(v, ijk[0], ijk[1], ijk[2])];
+          bad += prim_from_cons_cell(P, qc, &wl[std::size_t(g + 3) * neq]);
+        }
+        // reconstruction in cells i = -1..n: WL[i] -> face i+1/2, WR[i] -> face i-1/2
+        for (int i = -1; i <= n; ++i) {
+          for (int v = 0; v < neq; ++v) {
+            const T* c = &wl[std::size_t(i + 3) * neq + v];
+            T l, r;
+            if (P.recon == RECON_WENO5_JS) {
+              weno5_js(c[-2 * neq], c[-neq], c[0], c[neq], c[2 * neq], P.weno_eps, &l, &r);
+            } else {  // PAPER.md:155-157 piecewise constant
+              l = c[0]; r = c[0];
+            }
+            WL[std::size_t(i + 1) * neq + v] = l;
+            WR[std::size_t(i + 1) * neq + v] = r;
+          }
+        }
+        // faces f = i+1/2, i = -1..n-1: left state from cell i, right state from cell i+1
+        for (int i = -1; i < n; ++i)
+          bad += hllc_face(P, dir, &WL[std::size_t(i + 1) * neq], &WR[std::size_t(i + 2) * neq],
+                           &Ff[std::size_t(i + 1) * neq], &uf[i + 1]);
+        // eq.(10): flux difference and the alpha_i div(u) source with the cell-centre alpha_i
+        for (int i = 0; i < n; ++i) {
+          ijk[dir] = i;
+          for (int v = 0; v < neq; ++v) {
+            std::size_t t = idx(v, ijk[0], ijk[1], ijk[2]);
+            rhs_out[t] = rhs_out[t] + (Ff[std::size_t(i) * neq + v] - Ff[std::size_t(i + 1) * neq + v]) / P.dx[dir];
+          }
+          for (int f = 0; f < N; ++f) {
+            std::size_t t = idx(P.i_alpha(f), ijk[0], ijk[1], ijk[2]);
+            rhs_out[t] = rhs_out[t] + q[t] * (uf[i + 1] - uf[i]) / P.dx[dir];
+          }
+        }
+      }
+    }
+    return bad;
+  }
+
+  void clamp_all(T* q) const {
+    if (!P.clamp) return;
+    const int neq = P.neq();
+    const std::size_t nc = P.cells();
+#pragma omp parallel for schedule(static)
+    for (long c = 0; c < (long)nc; ++c) {
+      T qc[kMaxEq];
+      for (int v = 0; v < neq; ++v) qc[v] = q[std::size_t(v) * nc + c];
+      clamp_cell(P, qc);
+      for (int v = 0; v < neq; ++v) q[std::size_t(v) * nc + c] = qc[v];
+    }
+  }
+
+  // O6: one SSP-RK3 step, q updated in place.
+  long rk3_step(T* q, const T& dt) const {
+    const std::size_t tot = P.cells() * P.neq();
+    std::vector<T> q1(tot), L(tot);
+    long bad = 0;
+    bad += rhs(q, L.data());
+#pragma omp parallel for schedule(static)
+    for (long t = 0; t < (long)tot; ++t) q1[t] = q[t] + dt * L[t];
+    clamp_all(q1.data());
+    bad += rhs(q1.data(), L.data());
+#pragma omp parallel for schedule(static)
+    for (long t = 0; t < (long)tot; ++t) q1[t] = T(0.75) * q[t] + T(0.25) * (q1[t] + dt * L[t]);
+    clamp_all(q1.data());
+    bad += rhs(q1.data(), L.data());
+#pragma omp parallel for schedule(static)
+    for (long t = 0; t < (long)tot; ++t) q[t] = o_ratio<T>(1, 3) * q[t] + o_ratio<T>(2, 3) * (q1[t] + dt * L[t]);
+    clamp_all(q);
+    return bad;
+  }
+
+  // O7 / A9: dt = cfl / max_cells sum_d (|u_d| + c)/dx_d
+  T cfl_dt(const T* q, const T& cfl) const {
+    const int neq = P.neq(), N = P.nfluids;
+    const std::size_t nc = P.cells();
+    T smax = T(0);
+    for (std::size_t c = 0; c < nc; ++c) {
+      T qc[kMaxEq], w[kMaxEq];
+      for (int v = 0; v < neq; ++v) qc[v] = q[std::size_t(v) * nc + c];
+      prim_from_cons_cell(P, qc, w);
+      T rho = T(0), Gam = T(0), Pi = T(0);
+      for (int i = 0; i < N; ++i) rho = rho + w[P.i_arho(i)];
+      for (int i = 0; i < N; ++i) {
+        Gam = Gam + w[P.i_alpha(i)] * P.G(i);
+        Pi = Pi + w[P.i_alpha(i)] * P.P(i);
+      }
+      T cs = o_sqrt(sound_speed_sq(Gam, Pi, w[P.i_E()], rho));
+      T s = T(0);
+      for (int d = 0; d < P.ndim; ++d) s = s + (o_abs(w[P.i_mom(d)]) + cs) / P.dx[d];
+      smax = o_max(smax, s);
+    }
+    return cfl / smax;
+  }
+};
+
+}  // namespace mfc_oracle
