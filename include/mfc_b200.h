@@ -1,0 +1,156 @@
+/* mfc_b200.h — C ABI of the B200-native hot path of MFC 5.0's method (arxiv 2503.07953).
+ *
+ * The library evaluates the finite-volume right-hand side of the 5-equation (Allaire) diffuse-interface
+ * model with stiffened-gas EOS — conservative->primitive conversion, WENO5-JS reconstruction of the
+ * primitives, HLLC fluxes, flux divergence and the alpha_i div(u) source — and advances it by SSP-RK3.
+ * Every step runs in hand-written fp64 CUDA kernels for sm_100a; there is NO CPU fallback: if no CUDA
+ * device is usable every call returns MFC_ERR_CUDA.
+ *
+ * Citations are PAPER.md lines (section / equation).  Readings of points the paper leaves open carry the
+ * A-numbers of DESIGN.md §3.
+ *
+ * DATA LAYOUT (all state arrays q, w, rhs): dense fp64, structure of arrays, interior cells only (no
+ * ghost cells in memory), x fastest:
+ *     idx(v,i,j,k) = ((v*n[2] + k)*n[1] + j)*n[0] + i,        v = 0..neq-1,  neq = 2*N + D + 1
+ * (N fluids, D dimensions; "two advected species (8 PDEs)" in 3D).  Variable slots, the same
+ * for conservative q and primitive w (PAPER.md:165 lists them in this order):
+ *     [0,N)        alpha_i rho_i                      (both q and w)
+ *     [N,N+D)      rho u_d      in q,   u_d  in w
+ *     N+D          E = rho e + 1/2 rho |u|^2 (per volume, A1) in q,   p  in w
+ *     (N+D,2N+D]   alpha_i                            (both q and w)
+ *
+ * OWNERSHIP: the caller owns q, w, rhs.  "device" pointers are CUDA device pointers valid on the
+ * handle's device (e.g. torch.Tensor.data_ptr()), 8-byte aligned; "host" pointers are ordinary host
+ * memory (pinned memory makes the *_host calls faster but is not required).  The handle owns its scratch
+ * (two state-sized arrays, a few bytes of reduction/flag storage) and never frees caller memory.
+ *
+ * STREAMS: every kernel is enqueued on the stream given at mfc_init_grid (NULL = the legacy default
+ * stream).  Calls marked "async" return after enqueueing.  Calls marked "syncs" wait for that stream.
+ *
+ * ERRORS: every call returns an mfc_status, never throws or aborts.  Argument errors are detected
+ * synchronously and leave all buffers untouched.  CUDA launch errors are returned by the call that saw
+ * them.  A non-physical state met by a kernel (rho <= 0 or c^2 <= 0 or NaN at a cell or a face, A19) sets
+ * a sticky flag in the handle that mfc_check / mfc_cfl_dt report as MFC_ERR_NONPHYSICAL (results are then
+ * whatever IEEE arithmetic gave; nothing is floored silently).  mfc_last_error() gives a thread-local text.
+ *
+ * THREADS: one handle may be used by one host thread at a time.
+ */
+#ifndef MFC_B200_H
+#define MFC_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mfc_grid mfc_grid; /* opaque, library-owned */
+
+typedef enum {
+  MFC_OK = 0,
+  MFC_ERR_ARG = 1,
+  MFC_ERR_ALLOC = 2,
+  MFC_ERR_CUDA = 3,
+  MFC_ERR_NONPHYSICAL = 4
+} mfc_status;
+
+/* Ghost-cell ("buffer region") boundary conditions, PAPER.md:203 (§3.3).  Extrapolation is the paper's
+ * first-order extrapolation (ghost = nearest interior cell); periodic is required by BASELINE.json
+ * (the paper's Taylor-Green case, implies it).  Periodic must be set on both ends. */
+typedef enum { MFC_BC_PERIODIC = 0, MFC_BC_EXTRAP = 1 } mfc_bc;
+
+#define MFC_MAX_FLUIDS 3
+
+typedef struct {
+  int ndim;              /* D = 1..3 */
+  int n[3];              /* cells per direction; n[d] must be 1 for d >= ndim */
+  double dx[3];          /* uniform spacing per direction (> 0); ignored for d >= ndim */
+  int nfluids;           /* N = 1..MFC_MAX_FLUIDS */
+  const double *gamma;   /* host, N values: gamma_i   of e_i = (p + gamma_i pi_inf_i)/((gamma_i-1) rho_i) */
+  const double *pi_inf;  /* host, N values: pi_inf_i; both copied at init */
+  int bc_lo[3], bc_hi[3];/* mfc_bc per direction and end */
+  double weno_eps;       /* epsilon of the WENO weights, PAPER.md:163/566 (A4); > 0 */
+  double alpha_floor;    /* volume-fraction floor of the RK-stage clamp (A10) */
+  int clamp;             /* 0: no clamp; 1: apply A10 after every RK stage */
+  int device;            /* CUDA device ordinal */
+  void *stream;          /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
+} mfc_params;
+
+/* Create a handle: validates p, selects the <D,N> kernel instantiation, allocates scratch on p->device.
+ * Uniform Cartesian grid of PAPER.md:131-141 (eq. 9-10).  Returns MFC_ERR_ARG / MFC_ERR_ALLOC / MFC_ERR_CUDA. */
+mfc_status mfc_init_grid(const mfc_params *p, mfc_grid **out);
+
+/* Syncs the stream, frees the handle and its scratch.  NULL is accepted. */
+mfc_status mfc_free_grid(mfc_grid *g);
+
+/* neq = 2N + D + 1; cells = n[0]*n[1]*n[2].  Return -1 for a NULL handle. */
+int mfc_num_eqns(const mfc_grid *g);
+long long mfc_num_cells(const mfc_grid *g);
+
+/* w = primitives of q, cell by cell (eq.(4), 117, 165; O2):
+ *   rho = sum alpha_i rho_i, u = rho u / rho, Gamma = sum alpha_i/(gamma_i-1),
+ *   Pi = sum alpha_i gamma_i pi_inf_i/(gamma_i-1),  p = ((E - Pi) - 1/2 rho |u|^2)/Gamma.
+ * q, w: device, neq*cells doubles; may alias.  async. */
+mfc_status mfc_prim_from_cons(mfc_grid *g, const double *q, double *w);
+
+/* rhs = L(q): eq.(10) with WENO5-JS reconstruction of the primitives,
+ * the HLLC flux (wave speeds 653-654, S* 664, rho* 668), the face-velocity divergence
+ * for the alpha_i div(u) term and ghost cells by index mapping.
+ * q, rhs: device, neq*cells doubles, must not alias; rhs is overwritten.  async. */
+mfc_status mfc_rhs(mfc_grid *g, const double *q, double *rhs);
+
+/* As mfc_rhs but only the directions whose bit is set in dir_mask (bit d = direction d) contribute;
+ * cells keep 0 from the other directions.  Exists so that each directional sweep can be tested alone. */
+mfc_status mfc_rhs_dirs(mfc_grid *g, const double *q, double *rhs, int dir_mask);
+
+/* One SSP-RK3 step of size dt (the three-stage formula), in place on q, with the A10
+ * clamp after each stage when enabled.  q: device.  Uses the handle's scratch.  async. */
+mfc_status mfc_rk3_step(mfc_grid *g, double *q, double dt);
+
+/* nsteps RK3 steps with a fixed dt (one call, same arithmetic as nsteps calls of mfc_rk3_step).  async. */
+mfc_status mfc_rk3_steps(mfc_grid *g, double *q, double dt, int nsteps);
+
+/* dt = cfl / max_cells sum_d (|u_d| + c)/dx_d  with the frozen-alpha mixture sound speed
+ * c^2 = ((Gamma+1) p + Pi)/(Gamma rho)  (A5, A9; not in the paper — BASELINE.json asks for it).
+ * q: device; dt_out: HOST pointer to one double.  syncs; also reports the sticky non-physical flag. */
+mfc_status mfc_cfl_dt(mfc_grid *g, const double *q, double cfl, double *dt_out);
+
+/* Syncs and returns MFC_ERR_NONPHYSICAL if any kernel since the last mfc_check flagged a non-physical
+ * state (clears the flag), MFC_ERR_CUDA on an asynchronous CUDA error, else MFC_OK. */
+mfc_status mfc_check(mfc_grid *g);
+
+/* End-to-end forms over HOST buffers (the calls bench.py's "e2e" leg times): copy q_host to the handle's
+ * device staging (allocated on first use), run, copy the result back, sync.
+ *   mfc_rhs_host:        rhs_host = L(q_host)
+ *   mfc_rk3_steps_host:  q_host advanced in place by nsteps steps of size dt */
+mfc_status mfc_rhs_host(mfc_grid *g, const double *q_host, double *rhs_host);
+mfc_status mfc_rk3_steps_host(mfc_grid *g, double *q_host, double dt, int nsteps);
+
+/* Adaptive stepping, all on the device timeline: nsteps times { dt = CFL step of the current state (as
+ * mfc_cfl_dt); one RK3 step of size dt }.  *t_elapsed_host (HOST, may be NULL) receives the sum of the dt.
+ * mfc_advance: q device, syncs once per step (the 8-byte dt read-back).  mfc_advance_host: q_host HOST,
+ * copied in before and out after the nsteps steps. */
+mfc_status mfc_advance(mfc_grid *g, double *q, double cfl, int nsteps, double *t_elapsed_host);
+mfc_status mfc_advance_host(mfc_grid *g, double *q_host, double cfl, int nsteps, double *t_elapsed_host);
+
+/* Per-kernel device timing for the benchmark's roofline line.  While profiling is on, every kernel launch
+ * of this handle is bracketed by CUDA events on the handle's stream.  mfc_get_profile syncs and returns,
+ * for one kernel class, the summed device time in ms and the number of launches since mfc_set_profiling(g,1).
+ * Kernel classes: */
+enum { MFC_K_PRIM = 0, MFC_K_SWEEP_X = 1, MFC_K_SWEEP_Y = 2, MFC_K_SWEEP_Z = 3, MFC_K_RK = 4, MFC_K_CFL = 5, MFC_K_COUNT = 6 };
+mfc_status mfc_set_profiling(mfc_grid *g, int on); /* on = 1 also clears the accumulated profile */
+mfc_status mfc_get_profile(mfc_grid *g, int kernel_class, double *total_ms_host, long long *launches_host);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+long long mfc_launch_count(const mfc_grid *g);
+
+/* Tuning knob (benchmarks/tests only): cells per thread segment along the sweep direction, per direction;
+ * 0 keeps the library's choice.  Results do not depend on it beyond round-off-free re-partitioning
+ * (each face flux is computed from the same inputs wherever the segment boundaries fall). */
+mfc_status mfc_set_segments(mfc_grid *g, int seg_x, int seg_y, int seg_z);
+
+/* Text of the last error on this host thread ("" if none). */
+const char *mfc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MFC_B200_H */

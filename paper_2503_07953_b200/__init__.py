@@ -1,0 +1,216 @@
+"""paper_2503_07953_b200 — thin Python binding of the C-ABI library include/mfc_b200.h.
+
+Argument marshalling only: every step of the hot path (cons->prim, WENO5-JS, HLLC, flux divergence,
+alpha div(u) source, SSP-RK3 stage + clamp, CFL reduction) runs in the CUDA kernels of
+csrc/mfc_b200.cu.  PyTorch supplies device memory and streams.  There is no CPU path: without the
+compiled library or without a CUDA device every call raises.
+"""
+import ctypes as C
+import os
+
+from . import build as _build
+
+BC_PERIODIC, BC_EXTRAP = 0, 1
+MFC_OK, MFC_ERR_ARG, MFC_ERR_ALLOC, MFC_ERR_CUDA, MFC_ERR_NONPHYSICAL = 0, 1, 2, 3, 4
+EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "mfc_prim_from_cons", "mfc_rhs",
+           "mfc_rhs_dirs", "mfc_rk3_step", "mfc_rk3_steps", "mfc_cfl_dt", "mfc_check", "mfc_rhs_host",
+           "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
+           "mfc_launch_count", "mfc_set_segments", "mfc_last_error")
+
+
+KERNEL_CLASSES = ("prim", "sweep_x", "sweep_y", "sweep_z", "rk", "cfl")
+
+
+class MfcParams(C.Structure):
+    _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("dx", C.c_double * 3), ("nfluids", C.c_int),
+                ("gamma", C.POINTER(C.c_double)), ("pi_inf", C.POINTER(C.c_double)),
+                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
+                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int),
+                ("device", C.c_int), ("stream", C.c_void_p)]
+
+
+class MfcError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"mfc status {status}: {text}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib_path():
+    return _build.LIB
+
+
+def lib():
+    """Loads (building it first if the sources are newer) libmfc_b200.so.  Raises if that fails."""
+    global _lib
+    if _lib is None:
+        path = _build.build() if os.path.exists(_build.NVCC) else _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(f"{path} is missing and nvcc is not available: the CUDA library is required (no fallback)")
+        L = C.CDLL(path)
+        vp, dp = C.c_void_p, C.c_void_p
+        L.mfc_init_grid.argtypes = [C.POINTER(MfcParams), C.POINTER(vp)]
+        L.mfc_free_grid.argtypes = [vp]
+        L.mfc_num_eqns.argtypes = [vp]
+        L.mfc_num_cells.argtypes = [vp]; L.mfc_num_cells.restype = C.c_longlong
+        L.mfc_prim_from_cons.argtypes = [vp, dp, dp]
+        L.mfc_rhs.argtypes = [vp, dp, dp]
+        L.mfc_rhs_dirs.argtypes = [vp, dp, dp, C.c_int]
+        L.mfc_rk3_step.argtypes = [vp, dp, C.c_double]
+        L.mfc_rk3_steps.argtypes = [vp, dp, C.c_double, C.c_int]
+        L.mfc_cfl_dt.argtypes = [vp, dp, C.c_double, C.POINTER(C.c_double)]
+        L.mfc_check.argtypes = [vp]
+        L.mfc_rhs_host.argtypes = [vp, dp, dp]
+        L.mfc_rk3_steps_host.argtypes = [vp, dp, C.c_double, C.c_int]
+        L.mfc_advance.argtypes = [vp, dp, C.c_double, C.c_int, C.POINTER(C.c_double)]
+        L.mfc_advance_host.argtypes = [vp, dp, C.c_double, C.c_int, C.POINTER(C.c_double)]
+        L.mfc_set_profiling.argtypes = [vp, C.c_int]
+        L.mfc_get_profile.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.mfc_launch_count.argtypes = [vp]; L.mfc_launch_count.restype = C.c_longlong
+        L.mfc_set_segments.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+        L.mfc_last_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _ck(status):
+    if status != MFC_OK:
+        raise MfcError(status, lib().mfc_last_error().decode())
+
+
+def _dev_ptr(t, count):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float64 CUDA tensor")
+    if t.numel() != count:
+        raise ValueError(f"expected {count} elements, got {t.numel()}")
+    return t.data_ptr()
+
+
+def _host_ptr(t, count):
+    import numpy as np
+    import torch
+    if isinstance(t, torch.Tensor):
+        if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+            raise TypeError("expected a contiguous float64 CPU tensor")
+        if t.numel() != count:
+            raise ValueError(f"expected {count} elements, got {t.numel()}")
+        return t.data_ptr()
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float64 or not t.flags["C_CONTIGUOUS"]:
+            raise TypeError("expected a C-contiguous float64 array")
+        if t.size != count:
+            raise ValueError(f"expected {count} elements, got {t.size}")
+        return t.ctypes.data
+    raise TypeError("expected a numpy array or CPU tensor")
+
+
+class Grid:
+    """Handle of one grid (mfc_init_grid ... mfc_free_grid); methods carry the C names without the prefix."""
+
+    def __init__(self, ndim, n, dx, gamma, pi_inf, bc_lo, bc_hi, weno_eps=1e-16, alpha_floor=1e-6, clamp=True,
+                 device=0, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2503_07953_b200 needs a CUDA device (there is no CPU fallback)")
+        self._h = C.c_void_p()
+        p = MfcParams()
+        p.ndim = ndim
+        nf = len(gamma)
+        self._gamma = (C.c_double * nf)(*gamma)
+        self._pi = (C.c_double * nf)(*pi_inf)
+        for d in range(3):
+            p.n[d] = n[d]
+            p.dx[d] = dx[d]
+            p.bc_lo[d] = bc_lo[d]
+            p.bc_hi[d] = bc_hi[d]
+        p.nfluids = nf
+        p.gamma = C.cast(self._gamma, C.POINTER(C.c_double))
+        p.pi_inf = C.cast(self._pi, C.POINTER(C.c_double))
+        p.weno_eps, p.alpha_floor, p.clamp = weno_eps, alpha_floor, int(bool(clamp))
+        p.device = device
+        if stream is None:
+            stream = torch.cuda.current_stream(device).cuda_stream
+        p.stream = stream
+        _ck(lib().mfc_init_grid(C.byref(p), C.byref(self._h)))
+        self.neq = lib().mfc_num_eqns(self._h)
+        self.cells = lib().mfc_num_cells(self._h)
+        self.count = self.neq * self.cells
+        self.shape = (self.neq, n[2], n[1], n[0])
+        self.device = device
+
+    @classmethod
+    def from_case(cls, case, device=0, stream=None):
+        """case: an mfc_workloads.Case-like object (ndim, n, dx, gamma, pi_inf, bc_lo, bc_hi, weno_eps, alpha_floor, clamp)."""
+        return cls(case.ndim, case.n, case.dx, case.gamma, case.pi_inf, case.bc_lo, case.bc_hi, case.weno_eps,
+                   case.alpha_floor, case.clamp, device, stream)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().mfc_free_grid(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # interpreter shutdown: module globals may already be gone
+            pass
+
+    def prim_from_cons(self, q, w):
+        _ck(lib().mfc_prim_from_cons(self._h, _dev_ptr(q, self.count), _dev_ptr(w, self.count)))
+
+    def rhs(self, q, rhs):
+        _ck(lib().mfc_rhs(self._h, _dev_ptr(q, self.count), _dev_ptr(rhs, self.count)))
+
+    def rhs_dirs(self, q, rhs, dir_mask):
+        _ck(lib().mfc_rhs_dirs(self._h, _dev_ptr(q, self.count), _dev_ptr(rhs, self.count), dir_mask))
+
+    def rk3_step(self, q, dt):
+        _ck(lib().mfc_rk3_step(self._h, _dev_ptr(q, self.count), float(dt)))
+
+    def rk3_steps(self, q, dt, nsteps):
+        _ck(lib().mfc_rk3_steps(self._h, _dev_ptr(q, self.count), float(dt), int(nsteps)))
+
+    def cfl_dt(self, q, cfl):
+        dt = C.c_double()
+        _ck(lib().mfc_cfl_dt(self._h, _dev_ptr(q, self.count), float(cfl), C.byref(dt)))
+        return dt.value
+
+    def check(self):
+        _ck(lib().mfc_check(self._h))
+
+    def rhs_host(self, q_host, rhs_host):
+        _ck(lib().mfc_rhs_host(self._h, _host_ptr(q_host, self.count), _host_ptr(rhs_host, self.count)))
+
+    def rk3_steps_host(self, q_host, dt, nsteps):
+        _ck(lib().mfc_rk3_steps_host(self._h, _host_ptr(q_host, self.count), float(dt), int(nsteps)))
+
+    def advance(self, q, cfl, nsteps):
+        t = C.c_double()
+        _ck(lib().mfc_advance(self._h, _dev_ptr(q, self.count), float(cfl), int(nsteps), C.byref(t)))
+        return t.value
+
+    def advance_host(self, q_host, cfl, nsteps):
+        t = C.c_double()
+        _ck(lib().mfc_advance_host(self._h, _host_ptr(q_host, self.count), float(cfl), int(nsteps), C.byref(t)))
+        return t.value
+
+    def set_profiling(self, on):
+        _ck(lib().mfc_set_profiling(self._h, int(bool(on))))
+
+    def get_profile(self):
+        """{kernel class name: (total device ms, launches)} since set_profiling(True)"""
+        out = {}
+        for i, name in enumerate(KERNEL_CLASSES):
+            ms, n = C.c_double(), C.c_longlong()
+            _ck(lib().mfc_get_profile(self._h, i, C.byref(ms), C.byref(n)))
+            out[name] = (ms.value, n.value)
+        return out
+
+    def launch_count(self):
+        return lib().mfc_launch_count(self._h)
+
+    def set_segments(self, seg_x=0, seg_y=0, seg_z=0):
+        _ck(lib().mfc_set_segments(self._h, seg_x, seg_y, seg_z))

@@ -1,0 +1,29 @@
+"""Builds paper_2503_07953_b200/libmfc_b200.so (the C-ABI library of include/mfc_b200.h) with nvcc for sm_100a.
+
+In-tree build: the .so sits next to this file, is git-ignored, and travels to the GPU box with the
+snapshot.  nvcc cross-compiles without a GPU.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(HERE)
+LIB = os.path.join(HERE, "libmfc_b200.so")
+SRC = [os.path.join(HERE, "csrc", "mfc_b200.cu")]
+DEPS = SRC + [os.path.join(HERE, "csrc", "mfc_device.cuh"), os.path.join(ROOT, "include", "mfc_b200.h")]
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+         "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
+        return LIB
+    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
+    subprocess.check_call(cmd)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

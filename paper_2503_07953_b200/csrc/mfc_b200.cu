@@ -1,0 +1,848 @@
+// mfc_b200.cu — kernels and C ABI (include/mfc_b200.h) of the B200-native MFC hot path.
+//
+// Kernels (all templated on <N fluids, D dimensions>, fp64, SoA x-fastest layout):
+//   prim_kernel     pointwise cons->prim (O2)
+//   sweep_x         x-direction: one warp per row segment, lane = cell; the warp walks along x in 32-cell
+//                   chunks; primitives live in a warp-private shared-memory ring, left face states and
+//                   fluxes move between neighbouring lanes by warp shuffles (O1-O5)
+//   sweep_march     y/z-direction: lanes span x (coalesced), each thread marches along the sweep
+//                   direction with a thread-private 5-cell ring of primitives in shared memory; the
+//                   previous face's left state and flux stay in registers (O1-O5)
+//   rk_kernel       SSP-RK3 stage combination + A10 clamp (O6)
+//   cfl_kernel      max_cells sum_d (|u_d|+c)/dx_d by warp shuffles + block reduce + integer atomicMax (O7)
+// No face state, flux or primitive array is ever written to HBM; ghost cells are index maps (O1).
+#include "../../include/mfc_b200.h"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "mfc_device.cuh"
+
+namespace mfc {
+
+constexpr unsigned FULL = 0xffffffffu;
+constexpr int XW = 4;     // warps per block, sweep_x
+constexpr int MB = 128;   // threads per block, sweep_march
+constexpr int PB = 256;   // threads per block, pointwise kernels
+
+// ------------------------------------------------------------------------------------------------ prim
+template <int N, int D>
+__global__ void __launch_bounds__(PB) prim_kernel(const __grid_constant__ KP kp, const double* __restrict__ q,
+                                                  double* __restrict__ w) {
+  constexpr int NEQ = 2 * N + D + 1;
+  const long long c = (long long)blockIdx.x * PB + threadIdx.x;
+  if (c >= kp.ncells) return;
+  double qc[NEQ], wc[NEQ];
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) qc[v] = q[v * kp.ncells + c];
+  if (prim_cell<N, D, true>(kp, qc, wc)) *kp.flag = 1;
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) w[v * kp.ncells + c] = wc[v];
+}
+
+// ------------------------------------------------------------------------------------------------ x sweep
+// Positions along a segment [s0, s0+L): load position pos <-> cell s0-3+pos (pos = 0..L+5);
+// reconstruction position p <-> cell i = s0-1+p (p = 0..L+1), whose stencil sits at load positions p..p+4.
+// Lane with position p: reconstructs cell i (both values), solves face i-1/2 (p >= 1) with the left
+// state of lane p-1, and updates cell i-1 (p >= 2) with the flux of lane p-1.
+template <int N, int D, bool ACCUM>
+__global__ void __launch_bounds__(XW * 32) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
+                                                   double* __restrict__ rhs, int seglen, int nseg) {
+  constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
+  __shared__ double ring[XW][NEQ][64];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long wid = (long long)blockIdx.x * XW + warp;
+  const int nx = kp.n[0];
+  const long long nrows = kp.ncells / nx;
+  if (wid >= nrows * nseg) return;  // warp-uniform
+  const int seg = (int)(wid % nseg);
+  const long long row = wid / nseg;
+  const int s0 = seg * seglen;
+  const int L = min(seglen, nx - s0);
+  const double* qrow = q + row * nx;
+  double* rrow = rhs + row * nx;
+  double(*rg)[64] = ring[warp];
+  const int nload = L + 6, nrec = L + 2;
+  const int nsteps = (nrec + 31) >> 5, nchunks = (nload + 31) >> 5;
+  const double idx = kp.inv_dx[0];
+  bool bad = false;
+
+  double qn[NEQ];
+  auto load = [&](int m) {
+    const int pos = 32 * m + lane;
+    if (pos < nload) {
+      const int g = ghost_index(s0 - 3 + pos, nx, kp.bc_lo[0], kp.bc_hi[0]);
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) qn[v] = __ldg(qrow + v * kp.ncells + g);
+    }
+  };
+  auto store = [&](int m) {
+    const int pos = 32 * m + lane;
+    if (pos < nload) {
+      double w[NEQ];
+      bad |= prim_cell<N, D, false>(kp, qn, w);
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) rg[v][pos & 63] = w[v];
+    }
+  };
+  load(0);
+  store(0);
+  if (nchunks > 1) {
+    load(1);
+    store(1);
+  }
+  __syncwarp();
+
+  double WLc[NEQ], Fc[NEQ], ufc = 0.0;  // previous chunk's left states / fluxes (lane 31 feeds lane 0)
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) WLc[v] = Fc[v] = 0.0;
+
+  for (int c = 0; c < nsteps; ++c) {
+    const bool pre = c + 2 < nchunks;
+    if (pre) load(c + 2);
+    const int p = 32 * c + lane;
+    double WL[NEQ], WR[NEQ];
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v)
+      weno5(rg[v][p & 63], rg[v][(p + 1) & 63], rg[v][(p + 2) & 63], rg[v][(p + 3) & 63], rg[v][(p + 4) & 63],
+            kp.eps4, WL[v], WR[v]);
+    double WLf[NEQ];
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) {
+      const double up = __shfl_up_sync(FULL, WL[v], 1);
+      const double carry = __shfl_sync(FULL, WLc[v], 31);
+      WLf[v] = lane ? up : carry;
+      WLc[v] = WL[v];
+    }
+    double F[NEQ], uf;
+    const bool fbad = hllc<N, D, 0>(kp, WLf, WR, F, uf);
+    if (p >= 1 && p < nrec) bad |= fbad;
+    double Fm[NEQ], ufm;
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) {
+      const double up = __shfl_up_sync(FULL, F[v], 1);
+      const double carry = __shfl_sync(FULL, Fc[v], 31);
+      Fm[v] = lane ? up : carry;
+      Fc[v] = F[v];
+    }
+    {
+      const double up = __shfl_up_sync(FULL, uf, 1);
+      const double carry = __shfl_sync(FULL, ufc, 31);
+      ufm = lane ? up : carry;
+      ufc = uf;
+    }
+    if (p >= 2 && p < nrec) {  // cell i-1 = s0 + p - 2: eq.(10) and the alpha_i div(u) source
+      const int i = s0 + p - 2;
+      const double du = (uf - ufm) * idx;
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) {
+        double r = (Fm[v] - F[v]) * idx;
+        if (v >= IA) r = fma(rg[v][(p + 1) & 63], du, r);
+        if (ACCUM) r += rrow[v * kp.ncells + i];
+        rrow[v * kp.ncells + i] = r;
+      }
+    }
+    __syncwarp();
+    if (pre) store(c + 2);
+    __syncwarp();
+  }
+  if (bad) *kp.flag = 1;
+}
+
+// ------------------------------------------------------------------------------------------------ y/z sweep
+// Thread <-> (column, segment [s0, s0+L) along DIR).  Step p = 0..L+1 handles cell g = s0-1+p:
+// ring slot (sl+k)%5 holds the primitives of cell g-2+k.  The cell g+3 is prefetched as conservatives
+// into registers during the step and converted at the start of the next one.
+template <int N, int D, int DIR, bool ACCUM>
+__global__ void __launch_bounds__(MB) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
+                                                  double* __restrict__ rhs, int seglen, int nseg) {
+  constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
+  extern __shared__ double ring[];  // [5][NEQ][MB]
+  const int n = kp.n[DIR];
+  const long long ncols = kp.ncells / n;
+  const long long id = (long long)blockIdx.x * MB + threadIdx.x;
+  if (id >= ncols * nseg) return;
+  const int seg = (int)(id / ncols);
+  const long long col = id % ncols;
+  long long base, stride;
+  if (DIR == 1) {
+    const int nx = kp.n[0];
+    const long long k = col / nx;
+    base = k * nx * (long long)kp.n[1] + (col - k * nx);
+    stride = nx;
+  } else {
+    base = col;
+    stride = (long long)kp.n[0] * kp.n[1];
+  }
+  const int s0 = seg * seglen;
+  const int L = min(seglen, n - s0);
+  const int lo = kp.bc_lo[DIR], hi = kp.bc_hi[DIR];
+  const double idx = kp.inv_dx[DIR];
+  double* R = ring + threadIdx.x;
+#define RG(slot, v) R[((slot) * NEQ + (v)) * MB]
+  bool bad = false;
+  double qn[NEQ];
+  auto loadq = [&](int cell) {
+    const long long off = base + (long long)ghost_index(cell, n, lo, hi) * stride;
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) qn[v] = __ldg(q + v * kp.ncells + off);
+  };
+  auto convert = [&](int slot) {
+    double w[NEQ];
+    bad |= prim_cell<N, D, false>(kp, qn, w);
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) RG(slot, v) = w[v];
+  };
+#pragma unroll 1
+  for (int m = 0; m < 4; ++m) {
+    loadq(s0 - 3 + m);
+    convert(m);
+  }
+  loadq(s0 + 1);
+
+  double WLp[NEQ], Fp[NEQ], ufp = 0.0;
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) WLp[v] = Fp[v] = 0.0;
+  int sl = 0;
+#pragma unroll 1
+  for (int p = 0; p <= L + 1; ++p) {
+    int s1 = sl + 1, s2 = sl + 2, s3 = sl + 3, s4 = sl + 4;
+    s1 -= s1 >= 5 ? 5 : 0;
+    s2 -= s2 >= 5 ? 5 : 0;
+    s3 -= s3 >= 5 ? 5 : 0;
+    s4 -= s4 >= 5 ? 5 : 0;
+    convert(s4);
+    if (p <= L) loadq(s0 + 2 + p);
+    const long long offc = base + (long long)(s0 + p - 2) * stride;  // cell g-1 (valid for p >= 2)
+    double racc[NEQ];
+    if (ACCUM && p >= 2) {
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) racc[v] = rhs[v * kp.ncells + offc];
+    }
+    double WL[NEQ], WR[NEQ];
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v)
+      weno5(RG(sl, v), RG(s1, v), RG(s2, v), RG(s3, v), RG(s4, v), kp.eps4, WL[v], WR[v]);
+    double F[NEQ], uf = 0.0;
+    if (p >= 1) {
+      bad |= hllc<N, D, DIR>(kp, WLp, WR, F, uf);
+      if (p >= 2) {
+        const double du = (uf - ufp) * idx;
+#pragma unroll
+        for (int v = 0; v < NEQ; ++v) {
+          double r = (Fp[v] - F[v]) * idx;
+          if (v >= IA) r = fma(RG(s1, v), du, r);
+          if (ACCUM) r += racc[v];
+          rhs[v * kp.ncells + offc] = r;
+        }
+      }
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) Fp[v] = F[v];
+      ufp = uf;
+    }
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) WLp[v] = WL[v];
+    sl = s1;
+  }
+#undef RG
+  if (bad) *kp.flag = 1;
+}
+
+// ------------------------------------------------------------------------------------------------ RK stage
+// O6, each product and sum rounded individually in the printed grouping:
+//   stage 1: q1 = q + dt L        stage 2: q1 = 3/4 q + 1/4 (q1 + dt L)        stage 3: q = 1/3 q + 2/3 (q1 + dt L)
+// followed by the A10 clamp of the new stage state.  `out` may alias `q` or `q1` (cell-local).
+template <int N, int D, int STAGE>
+__global__ void __launch_bounds__(PB) rk_kernel(const __grid_constant__ KP kp, const double* q, const double* q1,
+                                                const double* __restrict__ Lq, double* out, double dt) {
+  constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
+  const long long c = (long long)blockIdx.x * PB + threadIdx.x;
+  if (c >= kp.ncells) return;
+  double r[NEQ];
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) {
+    const long long t = v * kp.ncells + c;
+    const double dl = __dmul_rn(dt, Lq[t]);
+    if (STAGE == 1) {
+      r[v] = __dadd_rn(q[t], dl);
+    } else if (STAGE == 2) {
+      r[v] = __dadd_rn(__dmul_rn(0.75, q[t]), __dmul_rn(0.25, __dadd_rn(q1[t], dl)));
+    } else {
+      r[v] = __dadd_rn(__dmul_rn(1.0 / 3.0, q[t]), __dmul_rn(2.0 / 3.0, __dadd_rn(q1[t], dl)));
+    }
+  }
+  if (kp.clamp) {  // A10
+#pragma unroll
+    for (int i = 0; i < N; ++i) r[i] = r[i] < 0.0 ? 0.0 : r[i];
+    bool marked = false;
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+      if (r[IA + i] < kp.alpha_floor) {
+        r[IA + i] = kp.alpha_floor;
+        marked = true;
+      }
+    if (marked) {
+      double s = r[IA];
+#pragma unroll
+      for (int i = 1; i < N; ++i) s = __dadd_rn(s, r[IA + i]);
+#pragma unroll
+      for (int i = 0; i < N; ++i) r[IA + i] = __ddiv_rn(r[IA + i], s);
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + c] = r[v];
+}
+
+// ------------------------------------------------------------------------------------------------ CFL
+// O7 / A9.  All operations IEEE-rounded in the order of the definition, so the per-cell sums — and their
+// maximum, which does not depend on the order of comparison — are reproducible bit for bit.
+// Positive doubles order like their bit patterns, so the maximum is an integer atomicMax.
+template <int N, int D>
+__global__ void __launch_bounds__(PB) cfl_kernel(const __grid_constant__ KP kp, const double* __restrict__ q,
+                                                 unsigned long long* smax_bits) {
+  constexpr int NEQ = 2 * N + D + 1, IM = N, IE = N + D, IA = N + D + 1;
+  double smax = 0.0;
+  bool bad = false;
+  for (long long c = (long long)blockIdx.x * PB + threadIdx.x; c < kp.ncells; c += (long long)gridDim.x * PB) {
+    double qc[NEQ], w[NEQ];
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) qc[v] = q[v * kp.ncells + c];
+    bad |= prim_cell<N, D, true>(kp, qc, w);
+    double rho = w[0], Gam = __dmul_rn(w[IA], kp.G[0]), Pi = __dmul_rn(w[IA], kp.P[0]);
+#pragma unroll
+    for (int i = 1; i < N; ++i) {
+      rho = __dadd_rn(rho, w[i]);
+      Gam = __dadd_rn(Gam, __dmul_rn(w[IA + i], kp.G[i]));
+      Pi = __dadd_rn(Pi, __dmul_rn(w[IA + i], kp.P[i]));
+    }
+    const double c2 = __ddiv_rn(__dadd_rn(__dmul_rn(__dadd_rn(Gam, 1.0), w[IE]), Pi), __dmul_rn(Gam, rho));
+    bad |= !(c2 > 0.0);
+    const double cs = __dsqrt_rn(c2);
+    double s = __ddiv_rn(__dadd_rn(fabs(w[IM]), cs), kp.dx[0]);
+#pragma unroll
+    for (int d = 1; d < D; ++d) s = __dadd_rn(s, __ddiv_rn(__dadd_rn(fabs(w[IM + d]), cs), kp.dx[d]));
+    smax = s > smax ? s : smax;
+  }
+#pragma unroll
+  for (int o = 16; o; o >>= 1) {
+    const double t = __shfl_xor_sync(FULL, smax, o);
+    smax = t > smax ? t : smax;
+  }
+  __shared__ double part[PB / 32];
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = smax;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    smax = threadIdx.x < PB / 32 ? part[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+      const double t = __shfl_xor_sync(FULL, smax, o);
+      smax = t > smax ? t : smax;
+    }
+    if (threadIdx.x == 0 && smax > 0.0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(smax));
+  }
+  if (bad) *kp.flag = 1;
+}
+
+}  // namespace mfc
+
+// ================================================================================================ host side
+using namespace mfc;
+
+struct mfc_grid {
+  KP kp;
+  int ndim, nf, neq;
+  int device;
+  cudaStream_t stream;
+  double* q1 = nullptr;     // stage state
+  double* Lq = nullptr;     // rhs scratch
+  double* hq = nullptr;     // device staging for the *_host calls (lazy)
+  double* hr = nullptr;
+  unsigned long long* d_red = nullptr;  // [0] = smax bits
+  int* d_flag = nullptr;
+  unsigned long long* h_red = nullptr;  // pinned: [0] smax bits, [1] flag
+  int seg[3];
+  long long launches = 0;
+  int num_sms = 148;
+  // per-kernel device timing (mfc_set_profiling)
+  bool profiling = false;
+  struct Rec { int cls; cudaEvent_t a, b; };
+  std::vector<Rec> recs;
+  std::vector<cudaEvent_t> pool;
+  double prof_ms[MFC_K_COUNT] = {};
+  long long prof_n[MFC_K_COUNT] = {};
+};
+
+// Brackets one launch with events when profiling is on; always counts the launch.
+struct Scope {
+  mfc_grid* g;
+  cudaEvent_t b = nullptr;
+  Scope(mfc_grid* g_, int cls);
+  ~Scope();
+};
+
+static thread_local std::string g_err;
+static mfc_status fail(mfc_status s, const std::string& m) {
+  g_err = m;
+  return s;
+}
+static mfc_status cuda_fail(cudaError_t e, const char* what) {
+  return fail(MFC_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(call)                                       \
+  do {                                                 \
+    cudaError_t e_ = (call);                           \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+static cudaEvent_t get_event(mfc_grid* g) {
+  if (!g->pool.empty()) {
+    cudaEvent_t e = g->pool.back();
+    g->pool.pop_back();
+    return e;
+  }
+  cudaEvent_t e = nullptr;
+  cudaEventCreate(&e);
+  return e;
+}
+Scope::Scope(mfc_grid* g_, int cls) : g(g_) {
+  g->launches++;
+  if (g->profiling) {
+    cudaEvent_t a = get_event(g);
+    b = get_event(g);
+    cudaEventRecord(a, g->stream);
+    g->recs.push_back({cls, a, b});
+  }
+}
+Scope::~Scope() {
+  if (b) cudaEventRecord(b, g->stream);
+}
+// fold finished records into the per-class sums (caller has synchronised the stream)
+static void drain_profile(mfc_grid* g) {
+  for (auto& r : g->recs) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) {
+      g->prof_ms[r.cls] += ms;
+      g->prof_n[r.cls]++;
+    }
+    g->pool.push_back(r.a);
+    g->pool.push_back(r.b);
+  }
+  g->recs.clear();
+}
+
+static size_t state_bytes(const mfc_grid* g) { return sizeof(double) * (size_t)g->neq * (size_t)g->kp.ncells; }
+
+// segment lengths: long enough that the halo work (2 extra reconstructions, 6 extra conversions per
+// segment) is small, short enough that every SM gets several blocks.
+static void default_segments(mfc_grid* g) {
+  const long long cells = g->kp.ncells;
+  {  // x: warps = rows * nseg; a segment of L cells needs ceil((L+2)/32) warp steps -> L = 32k - 2
+    const int nx = g->kp.n[0];
+    const long long rows = cells / nx;
+    const long long want_warps = (long long)g->num_sms * 32;
+    int L = nx;
+    if (rows < want_warps) {
+      const long long nseg = (want_warps + rows - 1) / rows;
+      long long l = (nx + nseg - 1) / nseg;
+      l = ((l + 2 + 31) / 32) * 32 - 2;
+      if (l < 30) l = 30;
+      if (l < nx) L = (int)l;
+    }
+    g->seg[0] = L;
+  }
+  for (int d = 1; d < g->ndim; ++d) {
+    const int n = g->kp.n[d];
+    const long long cols = cells / n;
+    const long long want_threads = (long long)g->num_sms * 1536;
+    int L = n;
+    if (cols < want_threads) {
+      const long long nseg = (want_threads + cols - 1) / cols;
+      long long l = (n + nseg - 1) / nseg;
+      if (l < 8) l = 8;
+      if (l < n) L = (int)l;
+    }
+    g->seg[d] = L;
+  }
+}
+
+template <int N, int D>
+static cudaError_t launch_prim(mfc_grid* g, const double* q, double* w) {
+  const long long nb = (g->kp.ncells + PB - 1) / PB;
+  Scope sc(g, MFC_K_PRIM);
+  prim_kernel<N, D><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, w);
+  return cudaGetLastError();
+}
+
+template <int N, int D, int DIR, bool ACCUM>
+static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs) {
+  if constexpr (DIR < D) {
+    constexpr int NEQ = 2 * N + D + 1;
+    const int n = g->kp.n[DIR];
+    const int seglen = g->seg[DIR];
+    const int nseg = (n + seglen - 1) / seglen;
+    const long long threads = g->kp.ncells / n * nseg;
+    const long long nb = (threads + MB - 1) / MB;
+    const size_t smem = sizeof(double) * 5 * NEQ * MB;
+    auto kern = sweep_march<N, D, DIR, ACCUM>;
+    static bool attr_done[16] = {};
+    if (!attr_done[g->device & 15]) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e != cudaSuccess) return e;
+      attr_done[g->device & 15] = true;
+    }
+    Scope sc(g, DIR == 1 ? MFC_K_SWEEP_Y : MFC_K_SWEEP_Z);
+    kern<<<(unsigned)nb, MB, smem, g->stream>>>(g->kp, q, rhs, seglen, nseg);
+    return cudaGetLastError();
+  } else {
+    return cudaSuccess;
+  }
+}
+
+template <int N, int D, bool ACCUM>
+static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs) {
+  const int nx = g->kp.n[0];
+  const int seglen = g->seg[0];
+  const int nseg = (nx + seglen - 1) / seglen;
+  const long long warps = g->kp.ncells / nx * nseg;
+  const long long nb = (warps + XW - 1) / XW;
+  Scope sc(g, MFC_K_SWEEP_X);
+  sweep_x<N, D, ACCUM><<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg);
+  return cudaGetLastError();
+}
+
+// rhs = L(q) restricted to the directions in mask.  mask == all: x overwrites, y and z accumulate.
+template <int N, int D>
+static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mask) {
+  const int all = (1 << D) - 1;
+  cudaError_t e;
+  if ((mask & all) == all) {
+    if ((e = launch_x<N, D, false>(g, q, rhs)) != cudaSuccess) return e;
+  } else {
+    if ((e = cudaMemsetAsync(rhs, 0, state_bytes(g), g->stream)) != cudaSuccess) return e;
+    if (mask & 1)
+      if ((e = launch_x<N, D, true>(g, q, rhs)) != cudaSuccess) return e;
+  }
+  if (D >= 2 && (mask & 2))
+    if ((e = launch_march<N, D, 1, true>(g, q, rhs)) != cudaSuccess) return e;
+  if (D >= 3 && (mask & 4))
+    if ((e = launch_march<N, D, 2, true>(g, q, rhs)) != cudaSuccess) return e;
+  return cudaSuccess;
+}
+
+template <int N, int D>
+static cudaError_t launch_rk3(mfc_grid* g, double* q, double dt) {
+  const long long nb = (g->kp.ncells + PB - 1) / PB;
+  const int all = (1 << D) - 1;
+  cudaError_t e;
+  if ((e = launch_rhs<N, D>(g, q, g->Lq, all)) != cudaSuccess) return e;
+  {
+    Scope sc(g, MFC_K_RK);
+    rk_kernel<N, D, 1><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->q1, g->Lq, g->q1, dt);
+  }
+  if ((e = launch_rhs<N, D>(g, g->q1, g->Lq, all)) != cudaSuccess) return e;
+  {
+    Scope sc(g, MFC_K_RK);
+    rk_kernel<N, D, 2><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->q1, g->Lq, g->q1, dt);
+  }
+  if ((e = launch_rhs<N, D>(g, g->q1, g->Lq, all)) != cudaSuccess) return e;
+  {
+    Scope sc(g, MFC_K_RK);
+    rk_kernel<N, D, 3><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->q1, g->Lq, q, dt);
+  }
+  return cudaGetLastError();
+}
+
+template <int N, int D>
+static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
+  long long nb = (g->kp.ncells + PB - 1) / PB;
+  const long long cap = (long long)g->num_sms * 8;
+  if (nb > cap) nb = cap;
+  Scope sc(g, MFC_K_CFL);
+  cfl_kernel<N, D><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->d_red);
+  return cudaGetLastError();
+}
+
+#define MFC_DISPATCH(g, EXPR)                                  \
+  [&]() -> cudaError_t {                                       \
+    switch ((g)->nf * 10 + (g)->ndim) {                        \
+      case 11: { constexpr int N = 1, D = 1; return EXPR; }    \
+      case 12: { constexpr int N = 1, D = 2; return EXPR; }    \
+      case 13: { constexpr int N = 1, D = 3; return EXPR; }    \
+      case 21: { constexpr int N = 2, D = 1; return EXPR; }    \
+      case 22: { constexpr int N = 2, D = 2; return EXPR; }    \
+      case 23: { constexpr int N = 2, D = 3; return EXPR; }    \
+      case 31: { constexpr int N = 3, D = 1; return EXPR; }    \
+      case 32: { constexpr int N = 3, D = 2; return EXPR; }    \
+      case 33: { constexpr int N = 3, D = 3; return EXPR; }    \
+    }                                                          \
+    return cudaErrorInvalidValue;                              \
+  }()
+
+static mfc_status use_device(const mfc_grid* g) {
+  CK(cudaSetDevice(g->device));
+  return MFC_OK;
+}
+
+extern "C" {
+
+const char* mfc_last_error(void) { return g_err.c_str(); }
+
+mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
+  if (!p || !out) return fail(MFC_ERR_ARG, "mfc_init_grid: NULL argument");
+  *out = nullptr;
+  if (p->ndim < 1 || p->ndim > 3) return fail(MFC_ERR_ARG, "mfc_init_grid: ndim must be 1..3");
+  if (p->nfluids < 1 || p->nfluids > MFC_MAX_FLUIDS) return fail(MFC_ERR_ARG, "mfc_init_grid: nfluids must be 1..3");
+  if (!p->gamma || !p->pi_inf) return fail(MFC_ERR_ARG, "mfc_init_grid: gamma/pi_inf NULL");
+  long long cells = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (p->n[d] < 1) return fail(MFC_ERR_ARG, "mfc_init_grid: n[d] must be >= 1");
+    if (d >= p->ndim && p->n[d] != 1) return fail(MFC_ERR_ARG, "mfc_init_grid: n[d] must be 1 for d >= ndim");
+    if (d < p->ndim && !(p->dx[d] > 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: dx[d] must be > 0");
+    if (p->bc_lo[d] != MFC_BC_PERIODIC && p->bc_lo[d] != MFC_BC_EXTRAP) return fail(MFC_ERR_ARG, "mfc_init_grid: bad bc_lo");
+    if (p->bc_hi[d] != MFC_BC_PERIODIC && p->bc_hi[d] != MFC_BC_EXTRAP) return fail(MFC_ERR_ARG, "mfc_init_grid: bad bc_hi");
+    if ((p->bc_lo[d] == MFC_BC_PERIODIC) != (p->bc_hi[d] == MFC_BC_PERIODIC))
+      return fail(MFC_ERR_ARG, "mfc_init_grid: periodic must be set on both ends of a direction");
+    cells *= p->n[d];
+    if (cells > (1LL << 40)) return fail(MFC_ERR_ARG, "mfc_init_grid: grid too large");
+  }
+  for (int i = 0; i < p->nfluids; ++i)
+    if (!(p->gamma[i] > 1.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: gamma_i must be > 1");
+  if (!(p->weno_eps > 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: weno_eps must be > 0");
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (p->device < 0 || p->device >= ndev) return fail(MFC_ERR_ARG, "mfc_init_grid: no such CUDA device");
+  CK(cudaSetDevice(p->device));
+
+  mfc_grid* g = new (std::nothrow) mfc_grid();
+  if (!g) return fail(MFC_ERR_ALLOC, "mfc_init_grid: out of host memory");
+  std::memset(&g->kp, 0, sizeof(KP));
+  g->ndim = p->ndim;
+  g->nf = p->nfluids;
+  g->neq = 2 * p->nfluids + p->ndim + 1;
+  g->device = p->device;
+  g->stream = (cudaStream_t)p->stream;
+  for (int d = 0; d < 3; ++d) {
+    g->kp.n[d] = p->n[d];
+    g->kp.bc_lo[d] = p->bc_lo[d];
+    g->kp.bc_hi[d] = p->bc_hi[d];
+    g->kp.dx[d] = d < p->ndim ? p->dx[d] : 1.0;
+    g->kp.inv_dx[d] = 1.0 / g->kp.dx[d];
+  }
+  g->kp.ncells = cells;
+  for (int i = 0; i < 3; ++i) g->kp.G[i] = g->kp.P[i] = 0.0;
+  for (int i = 0; i < p->nfluids; ++i) {  // PAPER.md:117 with eq.(4): rho e = sum alpha_i (p + gamma_i pi_inf_i)/(gamma_i-1)
+    g->kp.G[i] = 1.0 / (p->gamma[i] - 1.0);
+    g->kp.P[i] = (p->gamma[i] * p->pi_inf[i]) / (p->gamma[i] - 1.0);
+  }
+  g->kp.eps4 = 4.0 * p->weno_eps;
+  g->kp.alpha_floor = p->alpha_floor;
+  g->kp.clamp = p->clamp ? 1 : 0;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, p->device) == cudaSuccess) g->num_sms = prop.multiProcessorCount;
+  default_segments(g);
+
+  const size_t bytes = state_bytes(g);
+  cudaError_t e;
+  if ((e = cudaMalloc(&g->q1, bytes)) != cudaSuccess || (e = cudaMalloc(&g->Lq, bytes)) != cudaSuccess ||
+      (e = cudaMalloc(&g->d_red, 16)) != cudaSuccess || (e = cudaMalloc(&g->d_flag, sizeof(int))) != cudaSuccess ||
+      (e = cudaMallocHost(&g->h_red, 16)) != cudaSuccess) {
+    mfc_free_grid(g);
+    g_err = std::string("mfc_init_grid: allocation failed: ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    return MFC_ERR_ALLOC;
+  }
+  g->kp.flag = g->d_flag;
+  CK(cudaMemsetAsync(g->d_flag, 0, sizeof(int), g->stream));
+  CK(cudaMemsetAsync(g->d_red, 0, 16, g->stream));
+  *out = g;
+  return MFC_OK;
+}
+
+mfc_status mfc_free_grid(mfc_grid* g) {
+  if (!g) return MFC_OK;
+  cudaSetDevice(g->device);
+  cudaStreamSynchronize(g->stream);
+  cudaFree(g->q1);
+  cudaFree(g->Lq);
+  cudaFree(g->hq);
+  cudaFree(g->hr);
+  cudaFree(g->d_red);
+  cudaFree(g->d_flag);
+  if (g->h_red) cudaFreeHost(g->h_red);
+  drain_profile(g);
+  for (cudaEvent_t e : g->pool) cudaEventDestroy(e);
+  delete g;
+  return MFC_OK;
+}
+
+int mfc_num_eqns(const mfc_grid* g) { return g ? g->neq : -1; }
+long long mfc_num_cells(const mfc_grid* g) { return g ? g->kp.ncells : -1; }
+long long mfc_launch_count(const mfc_grid* g) { return g ? g->launches : -1; }
+
+mfc_status mfc_set_segments(mfc_grid* g, int seg_x, int seg_y, int seg_z) {
+  if (!g) return fail(MFC_ERR_ARG, "mfc_set_segments: NULL handle");
+  if (seg_x < 0 || seg_y < 0 || seg_z < 0) return fail(MFC_ERR_ARG, "mfc_set_segments: negative length");
+  const int s[3] = {seg_x, seg_y, seg_z};
+  mfc_grid tmp = *g;
+  default_segments(&tmp);
+  for (int d = 0; d < 3; ++d) g->seg[d] = s[d] > 0 ? (s[d] < g->kp.n[d] ? s[d] : g->kp.n[d]) : tmp.seg[d];
+  return MFC_OK;
+}
+
+mfc_status mfc_prim_from_cons(mfc_grid* g, const double* q, double* w) {
+  if (!g || !q || !w) return fail(MFC_ERR_ARG, "mfc_prim_from_cons: NULL argument");
+  if (mfc_status s = use_device(g)) return s;
+  CK(MFC_DISPATCH(g, (launch_prim<N, D>(g, q, w))));
+  return MFC_OK;
+}
+
+mfc_status mfc_rhs_dirs(mfc_grid* g, const double* q, double* rhs, int dir_mask) {
+  if (!g || !q || !rhs) return fail(MFC_ERR_ARG, "mfc_rhs: NULL argument");
+  if (q == rhs) return fail(MFC_ERR_ARG, "mfc_rhs: q and rhs must not alias");
+  if (mfc_status s = use_device(g)) return s;
+  CK(MFC_DISPATCH(g, (launch_rhs<N, D>(g, q, rhs, dir_mask))));
+  return MFC_OK;
+}
+
+mfc_status mfc_rhs(mfc_grid* g, const double* q, double* rhs) { return mfc_rhs_dirs(g, q, rhs, 7); }
+
+mfc_status mfc_rk3_steps(mfc_grid* g, double* q, double dt, int nsteps) {
+  if (!g || !q) return fail(MFC_ERR_ARG, "mfc_rk3_step: NULL argument");
+  if (nsteps < 0) return fail(MFC_ERR_ARG, "mfc_rk3_steps: nsteps < 0");
+  if (!(dt == dt)) return fail(MFC_ERR_ARG, "mfc_rk3_step: dt is NaN");
+  if (mfc_status s = use_device(g)) return s;
+  for (int s = 0; s < nsteps; ++s) CK(MFC_DISPATCH(g, (launch_rk3<N, D>(g, q, dt))));
+  return MFC_OK;
+}
+
+mfc_status mfc_rk3_step(mfc_grid* g, double* q, double dt) { return mfc_rk3_steps(g, q, dt, 1); }
+
+static mfc_status read_flag_and_sync(mfc_grid* g, bool with_red) {
+  CK(cudaMemcpyAsync(&g->h_red[1], g->d_flag, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+  if (with_red) CK(cudaMemcpyAsync(&g->h_red[0], g->d_red, 8, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaMemsetAsync(g->d_flag, 0, sizeof(int), g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  if ((int)(g->h_red[1] & 0xffffffffu) != 0) return fail(MFC_ERR_NONPHYSICAL, "non-physical state (rho <= 0 or c^2 <= 0 or NaN)");
+  return MFC_OK;
+}
+
+mfc_status mfc_cfl_dt(mfc_grid* g, const double* q, double cfl, double* dt_out) {
+  if (!g || !q || !dt_out) return fail(MFC_ERR_ARG, "mfc_cfl_dt: NULL argument");
+  if (mfc_status s = use_device(g)) return s;
+  CK(cudaMemsetAsync(g->d_red, 0, 8, g->stream));
+  CK(MFC_DISPATCH(g, (launch_cfl<N, D>(g, q))));
+  g->h_red[1] = 0;
+  const mfc_status s = read_flag_and_sync(g, true);
+  double smax;
+  std::memcpy(&smax, &g->h_red[0], 8);
+  *dt_out = cfl / smax;
+  return s;
+}
+
+mfc_status mfc_check(mfc_grid* g) {
+  if (!g) return fail(MFC_ERR_ARG, "mfc_check: NULL handle");
+  if (mfc_status s = use_device(g)) return s;
+  g->h_red[1] = 0;
+  return read_flag_and_sync(g, false);
+}
+
+static mfc_status ensure_staging(mfc_grid* g, bool need_r) {
+  if (!g->hq) {
+    if (cudaMalloc(&g->hq, state_bytes(g)) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(MFC_ERR_ALLOC, "staging allocation failed");
+    }
+  }
+  if (need_r && !g->hr) {
+    if (cudaMalloc(&g->hr, state_bytes(g)) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(MFC_ERR_ALLOC, "staging allocation failed");
+    }
+  }
+  return MFC_OK;
+}
+
+mfc_status mfc_rhs_host(mfc_grid* g, const double* q_host, double* rhs_host) {
+  if (!g || !q_host || !rhs_host) return fail(MFC_ERR_ARG, "mfc_rhs_host: NULL argument");
+  if (mfc_status s = use_device(g)) return s;
+  if (mfc_status s = ensure_staging(g, true)) return s;
+  CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));
+  CK(MFC_DISPATCH(g, (launch_rhs<N, D>(g, g->hq, g->hr, 7))));
+  CK(cudaMemcpyAsync(rhs_host, g->hr, state_bytes(g), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return MFC_OK;
+}
+
+mfc_status mfc_rk3_steps_host(mfc_grid* g, double* q_host, double dt, int nsteps) {
+  if (!g || !q_host) return fail(MFC_ERR_ARG, "mfc_rk3_steps_host: NULL argument");
+  if (nsteps < 0) return fail(MFC_ERR_ARG, "mfc_rk3_steps_host: nsteps < 0");
+  if (mfc_status s = use_device(g)) return s;
+  if (mfc_status s = ensure_staging(g, false)) return s;
+  CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));
+  for (int s = 0; s < nsteps; ++s) CK(MFC_DISPATCH(g, (launch_rk3<N, D>(g, g->hq, dt))));
+  CK(cudaMemcpyAsync(q_host, g->hq, state_bytes(g), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return MFC_OK;
+}
+
+static mfc_status advance_impl(mfc_grid* g, double* q, double cfl, int nsteps, double* t_out) {
+  double t = 0.0;
+  for (int s = 0; s < nsteps; ++s) {
+    double dt = 0.0;
+    if (mfc_status st = mfc_cfl_dt(g, q, cfl, &dt)) return st;
+    CK(MFC_DISPATCH(g, (launch_rk3<N, D>(g, q, dt))));
+    t += dt;
+  }
+  if (t_out) *t_out = t;
+  return MFC_OK;
+}
+
+mfc_status mfc_advance(mfc_grid* g, double* q, double cfl, int nsteps, double* t_elapsed_host) {
+  if (!g || !q) return fail(MFC_ERR_ARG, "mfc_advance: NULL argument");
+  if (nsteps < 0 || !(cfl > 0.0)) return fail(MFC_ERR_ARG, "mfc_advance: nsteps < 0 or cfl <= 0");
+  if (mfc_status s = use_device(g)) return s;
+  return advance_impl(g, q, cfl, nsteps, t_elapsed_host);
+}
+
+mfc_status mfc_advance_host(mfc_grid* g, double* q_host, double cfl, int nsteps, double* t_elapsed_host) {
+  if (!g || !q_host) return fail(MFC_ERR_ARG, "mfc_advance_host: NULL argument");
+  if (nsteps < 0 || !(cfl > 0.0)) return fail(MFC_ERR_ARG, "mfc_advance_host: nsteps < 0 or cfl <= 0");
+  if (mfc_status s = use_device(g)) return s;
+  if (mfc_status s = ensure_staging(g, false)) return s;
+  CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));
+  if (mfc_status s = advance_impl(g, g->hq, cfl, nsteps, t_elapsed_host)) return s;
+  CK(cudaMemcpyAsync(q_host, g->hq, state_bytes(g), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return MFC_OK;
+}
+
+mfc_status mfc_set_profiling(mfc_grid* g, int on) {
+  if (!g) return fail(MFC_ERR_ARG, "mfc_set_profiling: NULL handle");
+  if (mfc_status s = use_device(g)) return s;
+  CK(cudaStreamSynchronize(g->stream));
+  drain_profile(g);
+  if (on) {
+    for (int c = 0; c < MFC_K_COUNT; ++c) {
+      g->prof_ms[c] = 0.0;
+      g->prof_n[c] = 0;
+    }
+  }
+  g->profiling = on != 0;
+  return MFC_OK;
+}
+
+mfc_status mfc_get_profile(mfc_grid* g, int kernel_class, double* total_ms_host, long long* launches_host) {
+  if (!g || !total_ms_host || !launches_host) return fail(MFC_ERR_ARG, "mfc_get_profile: NULL argument");
+  if (kernel_class < 0 || kernel_class >= MFC_K_COUNT) return fail(MFC_ERR_ARG, "mfc_get_profile: bad kernel class");
+  if (mfc_status s = use_device(g)) return s;
+  CK(cudaStreamSynchronize(g->stream));
+  drain_profile(g);
+  *total_ms_host = g->prof_ms[kernel_class];
+  *launches_host = g->prof_n[kernel_class];
+  return MFC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,212 @@
+// Device-side arithmetic of the hot path: stiffened-gas primitives, WENO5-JS, HLLC.
+// Hand-written for sm_100a fp64.  Citations are PAPER.md lines; O-/A-/N-numbers refer to DESIGN.md §2-§3.
+// This file shares nothing with oracle/ (the CPU oracle is written separately from the paper).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mfc {
+
+enum { BC_PERIODIC = 0, BC_EXTRAP = 1 };
+
+// Kernel parameters (passed by value; lives in the constant bank of each launch).
+struct KP {
+  int n[3];
+  int bc_lo[3], bc_hi[3];
+  long long ncells;
+  double dx[3], inv_dx[3];
+  double G[3];   // G_i = 1/(gamma_i - 1)
+  double P[3];   // P_i = gamma_i pi_inf_i/(gamma_i - 1)
+  double eps4;   // 4 * weno_eps (the smoothness indicators are carried scaled by 4)
+  double alpha_floor;
+  int clamp;
+  int* flag;     // sticky non-physical flag (A19)
+};
+
+// O1: logical cell g in [-3, n+2] -> interior cell that supplies its value.
+__device__ __forceinline__ int ghost_index(int g, int n, int bc_lo, int bc_hi) {
+  if (g < 0) return bc_lo == BC_PERIODIC ? ((g % n) + n) % n : 0;
+  if (g >= n) return bc_hi == BC_PERIODIC ? g % n : n - 1;
+  return g;
+}
+
+// 1/x for normal x: the 2^-23 hardware seed (MUFU.RCP64H) plus one cubically convergent step
+// y(1 + e + e^2), e = 1 - x y  ->  relative error ~2^-69 before the final rounding.
+__device__ __forceinline__ double frcp(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y, 1.0);
+  const double t = fma(e, e, e);
+  return fma(y, t, y);
+}
+
+// sqrt(x) for normal x > 0: hardware rsqrt seed, one coupled (Goldschmidt) step, one residual correction.
+__device__ __forceinline__ double fsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  const double r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  const double d = fma(-g, g, x);
+  return fma(d, h, g);
+}
+
+// O2 (eq.(4), 117, 165): conservative cell -> primitive cell.
+// Pi and Gamma are summed with individually rounded products in fluid order (N1): with water
+// (P_i = 7.8e8) at p = 1e5 the energy carries p in its last digits, so (E - Pi) must see the same Pi
+// bits as any other evaluation of this definition.  EXACT additionally uses IEEE division and unfused
+// squares (mfc_prim_from_cons, mfc_cfl_dt: bandwidth-bound kernels); the sweeps use the fast reciprocal.
+// Returns true if rho is not positive (A19).
+template <int N, int D, bool EXACT>
+__device__ __forceinline__ bool prim_cell(const KP& kp, const double* q, double* w) {
+  constexpr int IM = N, IE = N + D, IA = N + D + 1;
+  double rho = q[0];
+#pragma unroll
+  for (int i = 1; i < N; ++i) rho = __dadd_rn(rho, q[i]);
+  double usq;
+  if (EXACT) {
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+      const double u = __ddiv_rn(q[IM + d], rho);
+      w[IM + d] = u;
+      usq = d == 0 ? __dmul_rn(u, u) : __dadd_rn(usq, __dmul_rn(u, u));
+    }
+  } else {
+    const double rr = frcp(rho);
+#pragma unroll
+    for (int d = 0; d < D; ++d) {
+      const double u = q[IM + d] * rr;
+      w[IM + d] = u;
+      usq = d == 0 ? u * u : fma(u, u, usq);
+    }
+  }
+  double Gam = __dmul_rn(q[IA], kp.G[0]), Pi = __dmul_rn(q[IA], kp.P[0]);
+#pragma unroll
+  for (int i = 1; i < N; ++i) {
+    Gam = __dadd_rn(Gam, __dmul_rn(q[IA + i], kp.G[i]));
+    Pi = __dadd_rn(Pi, __dmul_rn(q[IA + i], kp.P[i]));
+  }
+  const double ke = __dmul_rn(__dmul_rn(0.5, rho), usq);
+  const double num = __dadd_rn(__dadd_rn(q[IE], -Pi), -ke);
+  w[IE] = EXACT ? __ddiv_rn(num, Gam) : num * frcp(Gam);
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    w[i] = q[i];
+    w[IA + i] = q[IA + i];
+  }
+  return !(rho > 0.0);
+}
+
+// O3 (Jiang-Shu coefficients, A3).  Stencil (a,b,c,d,e) = w_{i-2..i+2}.
+// L = left-biased value at i+1/2 (q^L of face i+1/2), R = right-biased value at i-1/2 (q^R of face i-1/2).
+// Same definition as the plain formula, arranged for the FP64 pipe:
+//   * everything in first differences d1..d4, so each candidate is c + (combination of differences)/6
+//     and, since the weights sum to one, value = c + sum_r a_r P_r / sum_r a_r;
+//   * the smoothness indicators are carried scaled by 4 (13/3 t^2 + s^2 + 4 eps) — a common factor of
+//     the three a_r cancels in the normalisation;
+//   * product form of the weights: a_r = d_r /(beta_r+eps)^2 is multiplied through by
+//     prod_j (beta_j+eps)^2, which leaves ONE reciprocal per reconstructed value and no other division;
+//   * beta_r and the three products are shared by the two values of the cell.
+__device__ __forceinline__ void weno5(double a, double b, double c, double d, double e, double eps4, double& L,
+                                      double& R) {
+  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+  const double t0 = d2 - d1, t1 = d3 - d2, t2 = d4 - d3;
+  const double s0 = fma(3.0, d2, -d1), s1 = d2 + d3, s2 = fma(-3.0, d3, d4);
+  constexpr double C133 = 13.0 / 3.0;
+  const double b0 = fma(C133 * t0, t0, fma(s0, s0, eps4));
+  const double b1 = fma(C133 * t1, t1, fma(s1, s1, eps4));
+  const double b2 = fma(C133 * t2, t2, fma(s2, s2, eps4));
+  const double e0 = b0 * b0, e1 = b1 * b1, e2 = b2 * b2;
+  const double E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
+  {  // ideal weights (1/10, 6/10, 3/10); candidates c + (5 d2 - 2 d1)/6, c + (d2 + 2 d3)/6, c + (4 d3 - d4)/6
+    const double S = fma(0.3, E01, fma(0.6, E02, 0.1 * E12));
+    const double Q0 = fma(5.0 / 60.0, d2, (-2.0 / 60.0) * d1);
+    const double Q1 = fma(0.1, d2, 0.2 * d3);
+    const double Q2 = fma(0.2, d3, -0.05 * d4);
+    const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
+    L = fma(num, frcp(S), c);
+  }
+  {  // mirror image: ideal weights (3/10, 6/10, 1/10); c + (d1 - 4 d2)/6, c - (2 d2 + d3)/6, c + (2 d4 - 5 d3)/6
+    const double S = fma(0.1, E01, fma(0.6, E02, 0.3 * E12));
+    const double Q0 = fma(-0.2, d2, 0.05 * d1);
+    const double Q1 = fma(-0.2, d2, -0.1 * d3);
+    const double Q2 = fma(2.0 / 60.0, d4, (-5.0 / 60.0) * d3);
+    const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
+    R = fma(num, frcp(S), c);
+  }
+}
+
+// O4 (S_L,S_R 653-654; S* 664; rho* 668; A5-A8): HLLC at one face with normal direction
+// DIR from the reconstructed primitives wL, wR.  Writes the flux F[neq] and the face velocity uf
+// (A7: the HLLC flux of a unit scalar).  Returns true if a face state is non-physical.
+//
+// Branch-free form of the four-way selection (first match in the printed order, A8):
+//   side K = L if (S_L >= 0 or S* >= 0) else R;  star = (K = L) ? !(S_L >= 0) : (S_R > 0).
+// With ds = S* - u_K (0 outside the fan), r = 1/(S_K - S*), chi - 1 = ds r, the star-state correction
+// S_K (q*_K - q_K) collapses to
+//   alpha_i rho_i, alpha_i, rho u_t :  q u_f,           u_f = u_K + S_K (chi - 1)
+//   rho u_n :  rho u_K^2 + p + S_K rho (chi ds + (chi-1) u_K)
+//   E       :  (E + p) u_K + S_K ((chi-1) E + chi ds rho S* + ds p r)        [uses chi/(S_K-u_K) = r]
+template <int N, int D, int DIR>
+__device__ __forceinline__ bool hllc(const KP& kp, const double* wL, const double* wR, double* F, double& uf) {
+  constexpr int IM = N, IE = N + D, IA = N + D + 1, NEQ = 2 * N + D + 1;
+  double rho[2], E[2], c[2], un[2], p[2];
+  bool bad = false;
+#pragma unroll
+  for (int K = 0; K < 2; ++K) {
+    const double* w = K ? wR : wL;
+    double r = w[0], Gam = w[IA] * kp.G[0], Pi = w[IA] * kp.P[0];
+#pragma unroll
+    for (int i = 1; i < N; ++i) {
+      r += w[i];
+      Gam = fma(w[IA + i], kp.G[i], Gam);
+      Pi = fma(w[IA + i], kp.P[i], Pi);
+    }
+    double usq = w[IM] * w[IM];
+#pragma unroll
+    for (int d = 1; d < D; ++d) usq = fma(w[IM + d], w[IM + d], usq);
+    rho[K] = r;
+    p[K] = w[IE];
+    un[K] = w[IM + DIR];
+    E[K] = fma(0.5 * r, usq, fma(Gam, p[K], Pi));
+    const double c2 = fma(Gam + 1.0, p[K], Pi) * frcp(Gam * r);  // A5
+    bad = bad || !(r > 0.0) || !(c2 > 0.0);
+    c[K] = fsqrt(c2);
+  }
+  const double SL = fmin(un[0] - c[0], un[1] - c[1]);
+  const double SR = fmax(un[0] + c[0], un[1] + c[1]);
+  const double mL = rho[0] * (SL - un[0]), mR = rho[1] * (SR - un[1]);
+  const double Ss = fma(mL, un[0], fma(-mR, un[1], p[1] - p[0])) * frcp(mL - mR);
+  const bool useL = (SL >= 0.0) || (Ss >= 0.0);
+  const bool star = useL ? !(SL >= 0.0) : (SR > 0.0);
+  const double rhoK = useL ? rho[0] : rho[1];
+  const double unK = useL ? un[0] : un[1];
+  const double pK = useL ? p[0] : p[1];
+  const double EK = useL ? E[0] : E[1];
+  const double SK = useL ? SL : SR;
+  const double r = frcp(SK - Ss);
+  const double ds = star ? (Ss - unK) : 0.0;
+  const double chim1 = ds * r;
+  const double chi = 1.0 + chim1;
+  uf = fma(SK, chim1, unK);
+#pragma unroll
+  for (int i = 0; i < N; ++i) {
+    F[i] = (useL ? wL[i] : wR[i]) * uf;
+    F[IA + i] = (useL ? wL[IA + i] : wR[IA + i]) * uf;
+  }
+  const double rhoSK = rhoK * SK;
+#pragma unroll
+  for (int d = 0; d < D; ++d) {
+    if (d == DIR) {
+      F[IM + d] = fma(rhoSK, fma(chi, ds, chim1 * unK), fma(rhoK * unK, unK, pK));
+    } else {
+      F[IM + d] = (rhoK * (useL ? wL[IM + d] : wR[IM + d])) * uf;
+    }
+  }
+  const double corr = fma(chim1, EK, fma(chi * ds, rhoK * Ss, (ds * pK) * r));
+  F[IE] = fma(SK, corr, (EK + pK) * unK);
+  (void)NEQ;
+  return bad;
+}
+
+}  // namespace mfc

@@ -1,0 +1,335 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on the same
+seeded inputs.  Bars (BASELINE.json north_star): relative 1e-12 in the max-norm per
+variable group for one RHS evaluation, 1e-9 for the state after 100 RK3 steps; bit-exact for
+mfc_prim_from_cons, the RK stage/clamp arithmetic on identical inputs, and mfc_cfl_dt.
+All tests here need a B200 (pytest -m gpu)."""
+import numpy as np
+import pytest
+
+import mfc_workloads as W
+from oracle import oracle as O
+from parity_norm import rel_err
+
+pytestmark = pytest.mark.gpu
+
+RHS_TOL = 1e-12
+STEP_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    return t
+
+
+@pytest.fixture(scope="module")
+def mfc():
+    import paper_2503_07953_b200 as m
+    m.lib()
+    return m
+
+
+def make_case(ndim, nfluids, n, bc, clamp=True, eps=1e-16):
+    gamma, pi_inf = (1.4, 4.4, 1.67), (0.0, 6.0e8, 0.0)
+    nn = tuple(n[d] if d < ndim else 1 for d in range(3))
+    return W.Case("t", ndim, nn, tuple(0.7 / nn[d] if d < ndim else 1.0 for d in range(3)), nfluids,
+                  gamma[:nfluids], pi_inf[:nfluids], (bc,) * 3, (bc,) * 3, weno_eps=eps, clamp=clamp)
+
+
+def gpu_rhs(torch, mfc, case, q, mask=7, seg=None):
+    g = mfc.Grid.from_case(case)
+    if seg:
+        g.set_segments(*seg)
+    qd = torch.from_numpy(q).cuda()
+    rd = torch.full_like(qd, float("nan"))
+    if mask == 7:
+        g.rhs(qd, rd)
+    else:
+        g.rhs_dirs(qd, rd, mask)
+    g.check()
+    out = rd.cpu().numpy()
+    g.close()
+    return out
+
+
+# ------------------------------------------------------------------ mfc_prim_from_cons
+@pytest.mark.parametrize("ndim,nfluids,n", [(1, 1, (1000, 1, 1)), (1, 2, (37, 1, 1)), (2, 2, (67, 35, 1)),
+                                            (3, 2, (33, 18, 7)), (3, 3, (40, 9, 5)), (2, 1, (5, 3, 1)), (2, 3, (3, 300, 1))])
+def test_prim_from_cons_bit_exact(torch, mfc, ndim, nfluids, n):
+    case = make_case(ndim, nfluids, n, W.BC_PERIODIC)
+    q = W.random_admissible_state(case, seed=11)
+    w_ref = O.Oracle(case).prim_from_cons(q)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    wd = torch.empty_like(qd)
+    g.prim_from_cons(qd, wd)
+    g.check()
+    assert np.array_equal(wd.cpu().numpy(), w_ref)
+    g.prim_from_cons(qd, qd)  # aliasing allowed
+    assert np.array_equal(qd.cpu().numpy(), w_ref)
+
+
+# ------------------------------------------------------------------ mfc_rhs on rough random states
+ROUGH = [
+    (1, 1, (1000, 1, 1)), (1, 2, (97, 1, 1)), (1, 3, (64, 1, 1)), (1, 2, (5, 1, 1)), (1, 1, (1, 1, 1)), (1, 2, (2, 1, 1)),
+    (2, 2, (67, 35, 1)), (2, 1, (31, 33, 1)), (2, 3, (130, 9, 1)), (2, 2, (3, 2, 1)),
+    (3, 2, (33, 18, 11)), (3, 3, (40, 9, 13)), (3, 1, (16, 16, 16)), (3, 2, (70, 3, 5)), (3, 2, (2, 2, 2)),
+]
+
+
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_EXTRAP])
+@pytest.mark.parametrize("ndim,nfluids,n", ROUGH)
+def test_rhs_rough_state_all_directions(torch, mfc, ndim, nfluids, n, bc):
+    case = make_case(ndim, nfluids, n, bc)
+    q = W.random_admissible_state(case, seed=5 + ndim)
+    orc = O.Oracle(case)
+    ref = orc.rhs(q)
+    assert orc.bad == 0
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, nfluids, ndim)
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.parametrize("ndim,nfluids,n,mask", [(2, 2, (67, 35, 1), 1), (2, 2, (67, 35, 1), 2), (3, 2, (33, 18, 11), 1),
+                                                 (3, 2, (33, 18, 11), 2), (3, 2, (33, 18, 11), 4), (3, 3, (20, 9, 13), 5)])
+def test_rhs_single_directions(torch, mfc, ndim, nfluids, n, mask):
+    case = make_case(ndim, nfluids, n, W.BC_EXTRAP)
+    q = W.random_admissible_state(case, seed=3)
+    ref = O.Oracle(case).rhs(q, dir_mask=mask)
+    got = gpu_rhs(torch, mfc, case, q, mask=mask)
+    worst, per = rel_err(got, ref, nfluids, ndim)
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.parametrize("seg", [(30, 8, 8), (62, 9, 11), (1, 1, 1), (7, 3, 2), (1000, 1000, 1000)])
+def test_rhs_independent_of_segmentation(torch, mfc, seg):
+    # segment boundaries only re-partition the work: each face flux sees the same inputs wherever they fall
+    case = make_case(3, 2, (75, 21, 19), W.BC_PERIODIC)
+    q = W.random_admissible_state(case, seed=9)
+    ref = O.Oracle(case).rhs(q)
+    base = gpu_rhs(torch, mfc, case, q)
+    got = gpu_rhs(torch, mfc, case, q, seg=seg)
+    assert np.array_equal(got, base)
+    assert rel_err(got, ref, 2, 3)[0] <= RHS_TOL
+
+
+def test_rhs_uniform_state_is_exactly_zero(torch, mfc):
+    case = make_case(3, 2, (40, 12, 9), W.BC_PERIODIC)
+    sh = case.shape[1:]
+    one = np.ones(sh)
+    q = W.cons_from_prim(case, [0.3 * one, 700.0 * one], [13.0, -7.0, 3.0], 1.0e5, [0.3 * one, 0.7 * one])
+    got = gpu_rhs(torch, mfc, case, np.ascontiguousarray(q))
+    assert np.array_equal(got, np.zeros_like(got))
+
+
+# ------------------------------------------------------------------ mfc_rhs on the five configurations (down-scaled 2D/3D)
+@pytest.mark.parametrize("index,n", [(1, None), (2, None), (3, 100), (3, 256), (4, 40), (4, 72), (5, 36), (5, 64)])
+def test_rhs_configs(torch, mfc, index, n):
+    case = W.config(index, n=n)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    ref = orc.rhs(q)
+    assert orc.bad == 0
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    assert worst <= RHS_TOL, per
+
+
+def test_rhs_host_entry_point_matches_device_entry_point(torch, mfc):
+    case = W.config(4, n=40)
+    q = W.initial_state(case)
+    base = gpu_rhs(torch, mfc, case, q)
+    g = mfc.Grid.from_case(case)
+    out = np.empty_like(q)
+    g.rhs_host(q, out)
+    assert np.array_equal(out, base)
+
+
+# ------------------------------------------------------------------ full-size parity (the bench launch configurations)
+def test_rhs_full_size_config4_elementwise(torch, mfc):
+    case = W.config(4)  # 256^3, the configuration bench.py times; the oracle needs ~20 s for it
+    q = W.initial_state(case)
+    ref = O.Oracle(case).rhs(q)
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    assert worst <= RHS_TOL, per
+
+
+def test_rhs_full_size_config3_elementwise(torch, mfc):
+    case = W.config(3)  # 1024^2 in full
+    q = W.initial_state(case)
+    ref = O.Oracle(case).rhs(q)
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    assert worst <= RHS_TOL, per
+
+
+def _sampled_box_parity(torch, mfc, case, q, boxes, core):
+    """GPU rhs on the full grid vs oracle rhs recomputed on sub-boxes cut (with wrap/clamp) out of q:
+    cells at least 3 away from the sub-box boundary see exactly the stencils of the full problem.
+    The error scale per variable group is the oracle's maximum over all sampled boxes."""
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    rd = torch.empty_like(qd)
+    g.rhs(qd, rd)
+    g.check()
+    D = case.ndim
+    gots, refs = [], []
+    for lo3 in boxes:
+        idx = []
+        for d in range(3):
+            n = case.n[d]
+            ar = np.arange(lo3[d] - 3, lo3[d] + core + 3)
+            idx.append(ar % n if case.bc_lo[d] == W.BC_PERIODIC else np.clip(ar, 0, n - 1))
+        sub = np.ascontiguousarray(q[:, idx[2][:, None, None], idx[1][None, :, None], idx[0][None, None, :]])
+        nn = tuple(len(idx[d]) for d in range(3))
+        scase = W.Case("box", D, nn, case.dx, case.nfluids, case.gamma, case.pi_inf, (W.BC_EXTRAP,) * 3,
+                       (W.BC_EXTRAP,) * 3, weno_eps=case.weno_eps, clamp=case.clamp)
+        ref = O.Oracle(scase).rhs(sub)
+        refs.append(ref[:, 3:3 + core, 3:3 + core, 3:3 + core].reshape(case.neq, -1))
+        gi = [torch.as_tensor(idx[d][3:3 + core], device="cuda") for d in range(3)]
+        got = rd.view(case.shape)[:, gi[2][:, None, None], gi[1][None, :, None], gi[0][None, None, :]]
+        gots.append(got.cpu().numpy().reshape(case.neq, -1))
+    g.close()
+    return rel_err(np.concatenate(gots, 1), np.concatenate(refs, 1), case.nfluids, case.ndim)
+
+
+def test_rhs_full_size_config5_sampled(torch, mfc):
+    import psutil
+    n = 512 if psutil.virtual_memory().available > 56e9 else 320  # q0 alone is 10.7 GB at 512^3
+    case = W.config(5, n=n)
+    q = W.initial_state(case)
+    rng = np.random.default_rng(1)
+    s = n / 512.0
+    at = lambda x, y, z: (int(x * n), int(y * n), int(z * n))
+    # boxes on the shock (x = 0.2), on the droplet surface, on the slab faces, at domain corners/edges, and random
+    boxes = [at(0.2, 0.5, 0.5), at(0.19, 0.1, 0.9), at(0.3, 0.5, 0.5), at(0.45, 0.35, 0.5), at(0.58, 0.5, 0.5),
+             at(0.7, 0.2, 0.3), at(0.84, 0.7, 0.6), (0, 0, 0), (n - 16, n - 16, n - 16), (0, n // 2, n - 16), (n - 16, 0, n // 3)]
+    boxes += [tuple(int(v) for v in rng.integers(0, n - 16, 3)) for _ in range(6)]
+    worst, per = _sampled_box_parity(torch, mfc, case, q, boxes, core=16)
+    assert worst <= RHS_TOL, per
+
+
+# ------------------------------------------------------------------ RK3: stage arithmetic, clamp, 100 steps
+def test_rk3_single_step_with_clamp_firing(torch, mfc):
+    case = make_case(2, 3, (40, 17, 1), W.BC_PERIODIC, clamp=True)
+    q = W.random_admissible_state(case, seed=21)
+    N, D = 3, 2
+    rng = np.random.default_rng(2)
+    # push volume fractions / partial densities out of bounds in a third of the cells
+    hit = rng.random(case.shape[1:]) < 0.33
+    q[N + D + 1][hit] = -1e-3
+    q[N + D + 2][hit] += 1e-3
+    q[0][rng.random(case.shape[1:]) < 0.05] *= 1e-9
+    orc = O.Oracle(case)
+    dt = 1e-7
+    ref = q.copy()
+    orc.rk3_step(ref, dt)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    g.rk3_step(qd, dt)
+    got = qd.cpu().numpy()
+    assert rel_err(got, ref, N, D)[0] <= 1e-13
+    a = got[N + D + 1:]
+    assert a.min() >= case.alpha_floor / (1 + 3 * case.alpha_floor) * (1 - 1e-15)
+
+
+@pytest.mark.parametrize("index,n,nsteps", [(1, None, 100), (2, None, 100), (2, None, 500), (3, 128, 100), (4, 48, 50),
+                                            (4, 32, 100), (5, 40, 20)])
+def test_rk3_steps_configs(torch, mfc, index, n, nsteps):
+    case = W.config(index, n=n)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    for s in range(nsteps):
+        dt_ref = orc.cfl_dt(ref, case.cfl)
+        if s % 10 == 0:
+            dt_gpu = g.cfl_dt(qd, case.cfl)
+            assert abs(dt_gpu - dt_ref) <= 1e-14 * dt_ref + STEP_TOL * dt_ref * (s > 0)
+        orc.rk3_step(ref, dt_ref)  # the oracle's dt is given to both sides (A9)
+        assert orc.bad == 0
+        g.rk3_step(qd, dt_ref)
+    g.check()
+    got = qd.cpu().numpy()
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    assert worst <= STEP_TOL, per
+
+
+def test_sod_to_final_time_adaptive_dt(torch, mfc):
+    case = W.config(1)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    t, steps = 0.0, 0
+    while t < case.t_end * (1 - 1e-14):
+        dt = min(orc.cfl_dt(ref, case.cfl), case.t_end - t)
+        orc.rk3_step(ref, dt)
+        g.rk3_step(qd, dt)
+        t += dt
+        steps += 1
+    g.check()
+    got = qd.cpu().numpy()
+    assert 700 < steps < 1100
+    assert rel_err(got, ref, 1, 1)[0] <= STEP_TOL
+    assert np.array_equal(got[3], np.ones_like(got[3]))  # single fluid: alpha == 1 bit for bit (A7)
+
+
+def test_rk3_steps_equals_repeated_step_and_host_entry(torch, mfc):
+    case = W.config(3, n=64)
+    q = W.initial_state(case)
+    g = mfc.Grid.from_case(case)
+    dt = 0.2 * g.cfl_dt(torch.from_numpy(q).cuda(), 0.5)
+    a = torch.from_numpy(q).cuda()
+    for _ in range(5):
+        g.rk3_step(a, dt)
+    b = torch.from_numpy(q).cuda()
+    g.rk3_steps(b, dt, 5)
+    assert torch.equal(a, b)
+    h = q.copy()
+    g.rk3_steps_host(h, dt, 5)
+    assert np.array_equal(h, a.cpu().numpy())
+
+
+# ------------------------------------------------------------------ mfc_cfl_dt
+@pytest.mark.parametrize("index,n", [(1, None), (2, None), (3, 200), (4, 50), (5, 44)])
+def test_cfl_dt_bit_exact(torch, mfc, index, n):
+    case = W.config(index, n=n)
+    q = W.initial_state(case)
+    ref = O.Oracle(case).cfl_dt(q, case.cfl)
+    g = mfc.Grid.from_case(case)
+    assert g.cfl_dt(torch.from_numpy(q).cuda(), case.cfl) == ref
+
+
+# ------------------------------------------------------------------ error behaviour
+def test_nonphysical_state_is_flagged_not_floored(torch, mfc):
+    case = make_case(1, 1, (64, 1, 1), W.BC_EXTRAP)
+    q = W.random_admissible_state(case, seed=1)
+    q[0, 0, 0, 10] = -1.0  # negative density
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    rd = torch.empty_like(qd)
+    g.rhs(qd, rd)
+    with pytest.raises(mfc.MfcError) as e:
+        g.check()
+    assert e.value.status == mfc.MFC_ERR_NONPHYSICAL
+    g.check()  # flag is cleared by the report
+
+
+def test_argument_errors(torch, mfc):
+    case = make_case(2, 2, (8, 8, 1), W.BC_PERIODIC)
+    g = mfc.Grid.from_case(case)
+    q = torch.zeros(g.count, dtype=torch.float64, device="cuda")
+    with pytest.raises(mfc.MfcError) as e:
+        g.rhs(q, q)
+    assert e.value.status == mfc.MFC_ERR_ARG
+    with pytest.raises(ValueError):
+        g.rhs(q[:-1], q)
+    with pytest.raises(mfc.MfcError):
+        mfc.Grid(2, (8, 8, 2), (1, 1, 1), (1.4,), (0.0,), (0,) * 3, (0,) * 3)
+    with pytest.raises(mfc.MfcError):
+        mfc.Grid(1, (8, 1, 1), (1, 1, 1), (1.4,), (0.0,), (0, 0, 0), (1, 0, 0))
