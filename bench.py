@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py — grind time of the MFC hot path on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4|5|3|2|1] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over the whole grid: the CFL reduction (mfc_cfl_dt) followed by
+one SSP-RK3 step = 3 x (x/y/z sweeps: cons->prim, WENO5-JS, HLLC, flux divergence, alpha div(u) source)
++ 3 x (RK stage + clamp), through the C ABI (mfc_advance).  Metric: grind time = time / (RHS evaluations x
+cells x equations) in ns, RHS evaluations = 3 per step.
+
+Default workload: BASELINE.json configs[3] (3D periodic two-fluid mixing, 256^3, 8 equations — the shape of
+the paper's Table-1 benchmark case), seeded synthetic input (mfc_workloads).  The state arrays
+(1.07 GB each, 4 of them touched per step) are far larger than the 126 MB L2, so no L2 flush is needed.
+
+N > 1 (torchrun): the path runs on one GPU (north_star); ranks are independent replicas ("replicas only",
+DESIGN.md §9) — no data-path collective; time is the max over ranks, value the whole-job aggregate.
+
+--impl reference: the CPU oracle (oracle/), as it stands, on the host cores, on a bounded replica of the
+same workload; rank 0 only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "rhs_grind_time"
+UNIT = "ns/cell/eqn/rhs_eval"
+
+# Algorithmic flops per cell per RHS evaluation of the plain definition (add/sub, mul, div, sqrt = 1 flop
+# each), counted by the operation-counting instantiation of the oracle and extrapolated to n -> infinity
+# (tests/test_host_logic.py re-derives them).  Key: BASELINE.json config index.
+ALG_FLOPS_PER_CELL_RHS = {1: 557.0, 2: 810.0, 3: 1872.0, 4: 3186.0, 5: 3945.0}
+# FP64 peak "derived from unit counts and clocks": 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz.
+FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
+# DFMA-chain microbenchmark on this pool's B200: 17.05e12 DFMA/s = 34.1 TFLOP/s (SM clock ~1.80 GHz under FP64 load)
+FP64_PEAK_TFLOPS_MEASURED = 34.1
+
+
+def env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device):
+        self.device = device
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.device), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm_sorted = sorted(sm)
+        return {"sm_mhz": sm_sorted[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def reduce_max_ms(ms, world):
+    """max over ranks of a device-timed duration (every multi-GPU number is the slowest rank's)."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda" if dist.get_backend() == "nccl" else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def grind_ns(ms, steps, cells, neq, replicas=1):
+    """ns per cell per equation per RHS evaluation; 3 RHS evaluations per RK3 step; whole job = all replicas."""
+    return ms * 1e6 / (3.0 * steps * cells * neq * replicas)
+
+
+def sweep_alg_bytes_per_cell(kernel, neq, ndim):
+    """compulsory HBM bytes per cell of one sweep kernel in the three-sweep design:
+    x reads q and writes rhs; y and z read q, read rhs and write rhs."""
+    return (16 if kernel == "sweep_x" else 24) * neq
+
+
+def run_reference(args, rank):
+    """The oracle, as it stands, on the host cores: each step = one RK3 step (no CFL reduction: the oracle's
+    cfl_dt is serial) on a bounded replica of the workload."""
+    if rank != 0:
+        return
+    import mfc_workloads as W
+    from oracle import oracle as O
+    n_ref = {1: None, 2: None, 3: 256, 4: 64, 5: 56}[args.config]
+    case = W.config(args.config, n=n_ref)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    dt = orc.cfl_dt(q, case.cfl)
+    for _ in range(args.warmup):
+        orc.rk3_step(q, dt)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.rk3_step(q, dt)
+    sec = time.perf_counter() - t0
+    val = grind_ns(sec * 1e3, args.steps, case.cells, case.neq)
+    cores = O.num_threads()
+    sample = f"{args.steps} RK3 steps on a {'x'.join(str(v) for v in case.n[:case.ndim])} replica of config {args.config}"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3 / max(args.steps, 1), "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": case.name, "cells": case.cells, "neq": case.neq, "note": "CPU oracle on a bounded replica"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def cpu_baseline(config_index, budget_s=20.0):
+    import mfc_workloads as W
+    from oracle import oracle as O
+    n_ref = {1: None, 2: None, 3: 512, 4: 128, 5: 96}[config_index]
+    case = W.config(config_index, n=n_ref)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    dt = orc.cfl_dt(q, case.cfl)
+    t0 = time.perf_counter()
+    steps = 0
+    while steps < 2 or (time.perf_counter() - t0 < budget_s / 4 and steps < 50):
+        orc.rk3_step(q, dt)
+        steps += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    sec = time.perf_counter() - t0
+    return {"value": grind_ns(sec * 1e3, steps, case.cells, case.neq), "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{steps} RK3 steps ({3 * steps} RHS evaluations) on a {'x'.join(str(v) for v in case.n[:case.ndim])} "
+                      f"replica of config {config_index} ({sec:.1f} s of host time)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--n", type=int, default=None, help="override cells per direction (tests only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    rank, local_rank, world = env_int("RANK", 0), env_int("LOCAL_RANK", 0), env_int("WORLD_SIZE", 1)
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return 0
+
+    import numpy as np
+    import torch
+    import mfc_workloads as W
+    import paper_2503_07953_b200 as M
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    case = W.config(args.config, n=args.n)
+    q0 = W.initial_state(case)
+    g = M.Grid.from_case(case, device=local_rank)
+    qd = torch.from_numpy(q0).cuda()
+    cells, neq = case.cells, case.neq
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            torch.distributed.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident timing: the headline value
+    for _ in range(args.warmup):
+        g.advance(qd, case.cfl, 1)
+    g.check()
+    sampler = ClockSampler(local_rank)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = g.launch_count()
+    barrier()
+    sampler.start()
+    ev0.record()
+    g.advance(qd, case.cfl, args.steps)
+    ev1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    barrier()
+    launches = g.launch_count() - l0
+    ms = reduce_max_ms(ev0.elapsed_time(ev1), world)
+    g.check()
+    value = grind_ns(ms, args.steps, cells, neq, world)
+
+    # ---- per-kernel device times (CUDA events around every launch, on the launching stream) for the roofline
+    g.set_profiling(True)
+    g.advance(qd, case.cfl, args.steps)
+    prof = g.get_profile()
+    g.set_profiling(False)
+    tot_ms = sum(v[0] for v in prof.values())
+    kern = {k: {"ms_per_launch": v[0] / v[1], "launches_per_step": v[1] / args.steps, "share_of_step": v[0] / tot_ms}
+            for k, v in prof.items() if v[1]}
+    sweeps = [k for k in ("sweep_x", "sweep_y", "sweep_z") if k in kern]
+    dom = max(sweeps, key=lambda k: kern[k]["ms_per_launch"] * kern[k]["launches_per_step"])
+    dur_s = kern[dom]["ms_per_launch"] * 1e-3
+    flops_launch = ALG_FLOPS_PER_CELL_RHS[args.config] / case.ndim * cells
+    bytes_launch = sweep_alg_bytes_per_cell(dom, neq, case.ndim) * cells
+    hbm_peak, hbm_src = measured_peaks()
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu --set full capture
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get(f"config{args.config}", {}).get(dom)
+    roofline = {
+        "kernel": dom, "bound": "alu", "achieved": flops_launch / dur_s / 1e12, "peak": FP64_PEAK_TFLOPS_DERIVED,
+        "unit": "TFLOP/s", "frac": flops_launch / dur_s / 1e12 / FP64_PEAK_TFLOPS_DERIVED, "traffic": traffic,
+        "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md §8); DFMA microbenchmark measured "
+                       f"{FP64_PEAK_TFLOPS_MEASURED} TFLOP/s",
+        "frac_of_measured_dfma_peak": flops_launch / dur_s / 1e12 / FP64_PEAK_TFLOPS_MEASURED,
+        "alg_flops_per_launch": flops_launch, "alg_bytes_per_launch": bytes_launch, "ms_per_launch": dur_s * 1e3,
+        "hbm": {"achieved": bytes_launch / dur_s / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": bytes_launch / dur_s / 1e9 / hbm_peak,
+                "peak_source": hbm_src + " (MEASURED_PEAKS.json hbm_gbs)" if hbm_src == "measured" else "fallback of B200_PROFILING.md"},
+        "kernels": kern,
+    }
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the state, the step, D2H of the state, every step
+    e2e = None
+    if not args.no_e2e:
+        qh = torch.from_numpy(q0.copy()).pin_memory()
+        for _ in range(2):
+            g.advance_host(qh, case.cfl, 1)
+        n_e2e = max(2, min(args.steps, 10))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            g.advance_host(qh, case.cfl, 1)  # syncs inside
+        sec = time.perf_counter() - t0
+        e_ms = reduce_max_ms(sec * 1e3, world)
+        e2e = {"value": grind_ns(e_ms, n_e2e, cells, neq, world), "unit": UNIT, "h2d_bytes_per_step": 8 * neq * cells,
+               "d2h_bytes_per_step": 8 * neq * cells, "steps": n_e2e, "ms_per_step": e_ms / n_e2e,
+               "call": "mfc_advance_host(q_host pinned, cfl, 1) per step"}
+        del qh
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": case.name, "grid": list(case.n[:case.ndim]), "cells": cells, "neq": neq, "nfluids": case.nfluids,
+                   "rhs_evals_per_step": 3, "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "inputs larger than L2 (state array %.0f MB vs 126 MB L2)" % (8e-6 * neq * cells) if 8 * neq * cells > 3e8
+                   else "working set fits L2: latency/L2-bound configuration, roofline target does not apply"},
+        "cell_updates_per_s": cells * world * args.steps / (ms * 1e-3),
+        "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline,
+        "paper_context": "PAPER.md:720-726 Table 1 (other hardware, whole step): GH200 0.32, H100 SXM 0.38, A100 0.62 ns",
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(args.config)
+    if rank == 0:
+        print(json.dumps(out))
+    g.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

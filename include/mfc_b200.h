@@ -139,6 +139,16 @@ enum { MFC_K_PRIM = 0, MFC_K_SWEEP_X = 1, MFC_K_SWEEP_Y = 2, MFC_K_SWEEP_Z = 3, 
 mfc_status mfc_set_profiling(mfc_grid *g, int on); /* on = 1 also clears the accumulated profile */
 mfc_status mfc_get_profile(mfc_grid *g, int kernel_class, double *total_ms_host, long long *launches_host);
 
+/* Unit-level entry points of the two device functions every sweep kernel is built from (used by the parity
+ * tests to compare them one by one with the oracle's weno5_js / hllc_face; not needed by applications).
+ *   mfc_weno5_values: count stencils of 5 doubles each (stencil-major: s[5*t + k] = w_{i-2+k}) ->
+ *       left[t]  = left-biased value at i+1/2, right[t] = right-biased value at i-1/2
+ *   mfc_hllc_faces: count faces with reconstructed primitives wL, wR (face-major, neq values per face) ->
+ *       F (face-major, neq per face) and uf[count]; dir = face normal
+ * All pointers device; async. */
+mfc_status mfc_weno5_values(mfc_grid *g, const double *stencils, long long count, double *left, double *right);
+mfc_status mfc_hllc_faces(mfc_grid *g, int dir, const double *wL, const double *wR, long long count, double *F, double *uf);
+
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 long long mfc_launch_count(const mfc_grid *g);
 

@@ -253,14 +253,14 @@ def initial_state(case):
     return np.ascontiguousarray(_BUILDERS[case.builder](case))
 
 
-def random_admissible_state(case, seed=DEFAULT_SEED, rough=1.0):
+def random_admissible_state(case, seed=DEFAULT_SEED, rough=1.0, alpha_lo=0.05):
     """Seeded random admissible state (positive densities/pressure, alpha in bounds, sum alpha = 1):
     cell-wise independent values — the roughest possible input, used by unit parity tests."""
     rng = SplitMix64(seed)
     N, D = case.nfluids, case.ndim
     shape3 = case.shape[1:]
     cells = case.cells
-    raw = [rng.uniform(cells, 0.05, 1.0).reshape(shape3) for _ in range(N)]
+    raw = [rng.uniform(cells, alpha_lo, 1.0).reshape(shape3) for _ in range(N)]
     s = sum(raw)
     alpha = [_clip_alpha(case, r / s) for r in raw]
     s = sum(alpha)

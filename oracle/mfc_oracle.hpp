@@ -126,6 +126,13 @@ T sound_speed_sq(const T& Gam, const T& Pi, const T& p, const T& rho) {
 // O3 (Jiang-Shu coefficients of the paper's refs [30],[70], A3).
 // Stencil (a,b,c,d,e) = w_{i-2..i+2}.  *left = left-biased value at i+1/2 (q^L of
 // face i+1/2), *right = right-biased value at i-1/2 (q^R of face i-1/2).
+// Evaluation form (reading N2): PAPER.md:163 defines f = sum_r omega_r f^(r) with
+// sum_r omega_r = 1, hence f = c + sum_r omega_r (f^(r) - c); the candidate deviations f^(r) - c are
+// written in the first differences d1..d4 of the stencil:
+//   left :  (2a-7b+11c)/6 - c = (5 d2 - 2 d1)/6,  (-b+5c+2d)/6 - c = (d2 + 2 d3)/6,  (2c+5d-e)/6 - c = (4 d3 - d4)/6
+//   right:  (-a+5b+2c)/6 - c = (d1 - 4 d2)/6,     (2b+5c-d)/6 - c = -(2 d2 + d3)/6,  (11c-7d+2e)/6 - c = (2 d4 - 5 d3)/6
+// Same polynomials as the textbook form, but the rounding error is ~1/2 ulp of the value instead of 3-4 ulp
+// (pinned in tests/test_oracle_units.py against the 80-bit evaluation and against the textbook form).
 template <class T>
 void weno5_js(const T& a, const T& b, const T& c, const T& d, const T& e, const T& eps, T* left, T* right) {
   const T c1312 = o_ratio<T>(13, 12), c14 = o_ratio<T>(1, 4);
@@ -134,27 +141,28 @@ void weno5_js(const T& a, const T& b, const T& c, const T& d, const T& e, const 
   T b0 = c1312 * (t0 * t0) + c14 * (s0 * s0);
   T b1 = c1312 * (t1 * t1) + c14 * (s1 * s1);
   T b2 = c1312 * (t2 * t2) + c14 * (s2 * s2);
+  T d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
   // left-biased, ideal weights (1/10, 6/10, 3/10)
   {
-    T p0 = (T(2) * a - T(7) * b + T(11) * c) / T(6);
-    T p1 = (T(5) * c - b + T(2) * d) / T(6);
-    T p2 = (T(2) * c + T(5) * d - e) / T(6);
+    T P0 = (T(5) * d2 - T(2) * d1) / T(6);
+    T P1 = (d2 + T(2) * d3) / T(6);
+    T P2 = (T(4) * d3 - d4) / T(6);
     T a0 = o_ratio<T>(1, 10) / ((b0 + eps) * (b0 + eps));
     T a1 = o_ratio<T>(6, 10) / ((b1 + eps) * (b1 + eps));
     T a2 = o_ratio<T>(3, 10) / ((b2 + eps) * (b2 + eps));
     T s = a0 + a1 + a2;
-    *left = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+    *left = c + ((a0 / s) * P0 + (a1 / s) * P1 + (a2 / s) * P2);
   }
   // right-biased (mirror image), ideal weights (3/10, 6/10, 1/10), same beta
   {
-    T p0 = (T(5) * b - a + T(2) * c) / T(6);
-    T p1 = (T(2) * b + T(5) * c - d) / T(6);
-    T p2 = (T(11) * c - T(7) * d + T(2) * e) / T(6);
+    T P0 = (d1 - T(4) * d2) / T(6);
+    T P1 = (T(0) - (T(2) * d2 + d3)) / T(6);
+    T P2 = (T(2) * d4 - T(5) * d3) / T(6);
     T a0 = o_ratio<T>(3, 10) / ((b0 + eps) * (b0 + eps));
     T a1 = o_ratio<T>(6, 10) / ((b1 + eps) * (b1 + eps));
     T a2 = o_ratio<T>(1, 10) / ((b2 + eps) * (b2 + eps));
     T s = a0 + a1 + a2;
-    *right = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+    *right = c + ((a0 / s) * P0 + (a1 / s) * P1 + (a2 / s) * P2);
   }
 }
 
@@ -187,32 +195,40 @@ int hllc_face(const Params<T>& P, int dir, const T* wL, const T* wR, T* F, T* uf
   const T SR = o_max(un[0] + c[0], un[1] + c[1]);
   const T Sstar = (p[1] - p[0] + rho[0] * un[0] * (SL - un[0]) - rho[1] * un[1] * (SR - un[1])) /
                   (rho[0] * (SL - un[0]) - rho[1] * (SR - un[1]));
-  // physical flux and conservative state of side K, then the star correction S_K (q*_K - q_K)
+  // physical flux of side K, then the star correction S_K (q*_K - q_K).
+  // Evaluation form (reading N3): with chi = (S_K - u_K)/(S_K - S*) the jump q*_K - q_K is written
+  // out per component with  chi - 1 = (S* - u_K)/(S_K - S*)  formed directly,
+  //   alpha_i rho_i, alpha_i, rho u_t :  (chi - 1) q_K
+  //   rho u_n                         :  chi rho_K S* - rho_K u_K = rho_K ((chi - 1) S* + (S* - u_K))
+  //   E                               :  (chi - 1) E_K + chi (S* - u_K)(rho_K S* + p_K/(S_K - u_K))
+  // instead of forming q*_K and subtracting q_K: the same algebra, without the cancellation of two numbers of
+  // size |q| (7.8e8 for the energy of water) whose difference is of size |q| * Mach.
   auto side_flux = [&](int K, bool star, const T& SK) {
     const T chi = star ? (SK - un[K]) / (SK - Sstar) : T(1);
+    const T chim1 = star ? (Sstar - un[K]) / (SK - Sstar) : T(0);
     for (int v = 0; v < neq; ++v) F[v] = T(0);
     for (int i = 0; i < N; ++i) {
       T qv = w[K][P.i_arho(i)];
       F[P.i_arho(i)] = qv * un[K];
-      if (star) F[P.i_arho(i)] = F[P.i_arho(i)] + SK * (chi * qv - qv);
+      if (star) F[P.i_arho(i)] = F[P.i_arho(i)] + SK * (chim1 * qv);
       T av = w[K][P.i_alpha(i)];
       F[P.i_alpha(i)] = av * un[K];
-      if (star) F[P.i_alpha(i)] = F[P.i_alpha(i)] + SK * (chi * av - av);  // A7
+      if (star) F[P.i_alpha(i)] = F[P.i_alpha(i)] + SK * (chim1 * av);  // A7
     }
     for (int d = 0; d < D; ++d) {
       T qv = rho[K] * w[K][P.i_mom(d)];
       F[P.i_mom(d)] = qv * un[K] + (d == dir ? p[K] : T(0));
       if (star) {
-        T qs = (d == dir) ? chi * rho[K] * Sstar : chi * qv;
-        F[P.i_mom(d)] = F[P.i_mom(d)] + SK * (qs - qv);
+        T dq = (d == dir) ? rho[K] * (chim1 * Sstar + (Sstar - un[K])) : chim1 * qv;
+        F[P.i_mom(d)] = F[P.i_mom(d)] + SK * dq;
       }
     }
     F[P.i_E()] = (E[K] + p[K]) * un[K];
     if (star) {
-      T Es = chi * (E[K] + (Sstar - un[K]) * (rho[K] * Sstar + p[K] / (SK - un[K])));
-      F[P.i_E()] = F[P.i_E()] + SK * (Es - E[K]);
+      T dE = chim1 * E[K] + chi * ((Sstar - un[K]) * (rho[K] * Sstar + p[K] / (SK - un[K])));
+      F[P.i_E()] = F[P.i_E()] + SK * dE;
     }
-    *uf = star ? un[K] + SK * (chi - T(1)) : un[K];  // HLLC flux of a unit scalar (A7)
+    *uf = star ? un[K] + SK * chim1 : un[K];  // HLLC flux of a unit scalar (A7)
   };
   // first match in the printed order (A8)
   if (SL >= T(0)) side_flux(0, false, SL);

@@ -115,6 +115,14 @@ void oracle_weno5_js(const double* s, double eps, double* left, double* right) {
   weno5_js<double>(s[0], s[1], s[2], s[3], s[4], eps, left, right);
 }
 
+// the same text in 80-bit arithmetic, result rounded to double (pins the rounding error of the fp64 form, N2)
+void oracle_weno5_js_ld(const double* s, double eps, double* left, double* right) {
+  long double l, r;
+  weno5_js<long double>(s[0], s[1], s[2], s[3], s[4], (long double)eps, &l, &r);
+  *left = double(l);
+  *right = double(r);
+}
+
 int oracle_hllc_face(const oracle_params* p, int dir, const double* wL, const double* wR, double* F, double* uf) {
   return hllc_face<double>(convert<double>(p), dir, wL, wR, F, uf);
 }

@@ -41,6 +41,7 @@ def lib():
         L.oracle_rk3_step.argtypes = [pp, dp, C.c_double]; L.oracle_rk3_step.restype = C.c_long
         L.oracle_cfl_dt.argtypes = [pp, dp, C.c_double]; L.oracle_cfl_dt.restype = C.c_double
         L.oracle_weno5_js.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js.restype = None
+        L.oracle_weno5_js_ld.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js_ld.restype = None
         L.oracle_hllc_face.argtypes = [pp, C.c_int, dp, dp, dp, dp]
         L.oracle_clamp_cell.argtypes = [pp, dp]; L.oracle_clamp_cell.restype = None
         L.oracle_rhs_ld.argtypes = [pp, dp, dp, C.c_int]; L.oracle_rhs_ld.restype = C.c_long
@@ -134,6 +135,13 @@ def weno5_js(s, eps):
     s = np.ascontiguousarray(s, dtype=np.float64)
     l, r = C.c_double(), C.c_double()
     lib().oracle_weno5_js(_dp(s), float(eps), C.byref(l), C.byref(r))
+    return l.value, r.value
+
+
+def weno5_js_ld(s, eps):
+    s = np.ascontiguousarray(s, dtype=np.float64)
+    l, r = C.c_double(), C.c_double()
+    lib().oracle_weno5_js_ld(_dp(s), float(eps), C.byref(l), C.byref(r))
     return l.value, r.value
 
 

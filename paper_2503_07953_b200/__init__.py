@@ -15,7 +15,7 @@ MFC_OK, MFC_ERR_ARG, MFC_ERR_ALLOC, MFC_ERR_CUDA, MFC_ERR_NONPHYSICAL = 0, 1, 2,
 EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "mfc_prim_from_cons", "mfc_rhs",
            "mfc_rhs_dirs", "mfc_rk3_step", "mfc_rk3_steps", "mfc_cfl_dt", "mfc_check", "mfc_rhs_host",
            "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
-           "mfc_launch_count", "mfc_set_segments", "mfc_last_error")
+           "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error")
 
 
 KERNEL_CLASSES = ("prim", "sweep_x", "sweep_y", "sweep_z", "rk", "cfl")
@@ -68,6 +68,8 @@ def lib():
         L.mfc_advance_host.argtypes = [vp, dp, C.c_double, C.c_int, C.POINTER(C.c_double)]
         L.mfc_set_profiling.argtypes = [vp, C.c_int]
         L.mfc_get_profile.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+        L.mfc_weno5_values.argtypes = [vp, dp, C.c_longlong, dp, dp]
+        L.mfc_hllc_faces.argtypes = [vp, C.c_int, dp, dp, C.c_longlong, dp, dp]
         L.mfc_launch_count.argtypes = [vp]; L.mfc_launch_count.restype = C.c_longlong
         L.mfc_set_segments.argtypes = [vp, C.c_int, C.c_int, C.c_int]
         L.mfc_last_error.restype = C.c_char_p
@@ -208,6 +210,15 @@ class Grid:
             _ck(lib().mfc_get_profile(self._h, i, C.byref(ms), C.byref(n)))
             out[name] = (ms.value, n.value)
         return out
+
+    def weno5_values(self, stencils, left, right):
+        n = left.numel()
+        _ck(lib().mfc_weno5_values(self._h, _dev_ptr(stencils, 5 * n), n, _dev_ptr(left, n), _dev_ptr(right, n)))
+
+    def hllc_faces(self, direction, wL, wR, F, uf):
+        n = uf.numel()
+        _ck(lib().mfc_hllc_faces(self._h, int(direction), _dev_ptr(wL, n * self.neq), _dev_ptr(wR, n * self.neq), n,
+                                 _dev_ptr(F, n * self.neq), _dev_ptr(uf, n)))
 
     def launch_count(self):
         return lib().mfc_launch_count(self._h)

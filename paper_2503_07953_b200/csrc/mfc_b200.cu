@@ -346,6 +346,36 @@ __global__ void __launch_bounds__(PB) cfl_kernel(const __grid_constant__ KP kp, 
   if (bad) *kp.flag = 1;
 }
 
+// ------------------------------------------------------------------------------------------------ unit entry points
+__global__ void __launch_bounds__(PB) weno5_unit_kernel(const __grid_constant__ KP kp, const double* __restrict__ s,
+                                                        long long count, double* left, double* right) {
+  const long long t = (long long)blockIdx.x * PB + threadIdx.x;
+  if (t >= count) return;
+  double L, R;
+  weno5(s[5 * t], s[5 * t + 1], s[5 * t + 2], s[5 * t + 3], s[5 * t + 4], kp.eps4, L, R);
+  left[t] = L;
+  right[t] = R;
+}
+
+template <int N, int D, int DIR>
+__global__ void __launch_bounds__(PB) hllc_unit_kernel(const __grid_constant__ KP kp, const double* __restrict__ wL,
+                                                       const double* __restrict__ wR, long long count, double* F,
+                                                       double* uf) {
+  constexpr int NEQ = 2 * N + D + 1;
+  const long long t = (long long)blockIdx.x * PB + threadIdx.x;
+  if (t >= count) return;
+  double l[NEQ], r[NEQ], f[NEQ], u;
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) {
+    l[v] = wL[t * NEQ + v];
+    r[v] = wR[t * NEQ + v];
+  }
+  if (hllc<N, D, DIR>(kp, l, r, f, u)) *kp.flag = 1;
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) F[t * NEQ + v] = f[v];
+  uf[t] = u;
+}
+
 }  // namespace mfc
 
 // ================================================================================================ host side
@@ -552,6 +582,19 @@ static cudaError_t launch_rk3(mfc_grid* g, double* q, double dt) {
     Scope sc(g, MFC_K_RK);
     rk_kernel<N, D, 3><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->q1, g->Lq, q, dt);
   }
+  return cudaGetLastError();
+}
+
+template <int N, int D>
+static cudaError_t launch_hllc_unit(mfc_grid* g, int dir, const double* wL, const double* wR, long long count, double* F,
+                                    double* uf) {
+  const long long nb = (count + PB - 1) / PB;
+  Scope sc(g, MFC_K_PRIM);
+  if (dir == 0) hllc_unit_kernel<N, D, 0><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, wL, wR, count, F, uf);
+  if constexpr (D >= 2)
+    if (dir == 1) hllc_unit_kernel<N, D, 1><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, wL, wR, count, F, uf);
+  if constexpr (D >= 3)
+    if (dir == 2) hllc_unit_kernel<N, D, 2><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, wL, wR, count, F, uf);
   return cudaGetLastError();
 }
 
@@ -816,6 +859,28 @@ mfc_status mfc_advance_host(mfc_grid* g, double* q_host, double cfl, int nsteps,
   if (mfc_status s = advance_impl(g, g->hq, cfl, nsteps, t_elapsed_host)) return s;
   CK(cudaMemcpyAsync(q_host, g->hq, state_bytes(g), cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
+  return MFC_OK;
+}
+
+mfc_status mfc_weno5_values(mfc_grid* g, const double* stencils, long long count, double* left, double* right) {
+  if (!g || !stencils || !left || !right) return fail(MFC_ERR_ARG, "mfc_weno5_values: NULL argument");
+  if (count < 0) return fail(MFC_ERR_ARG, "mfc_weno5_values: count < 0");
+  if (mfc_status s = use_device(g)) return s;
+  if (count == 0) return MFC_OK;
+  {
+    Scope sc(g, MFC_K_PRIM);
+    weno5_unit_kernel<<<(unsigned)((count + PB - 1) / PB), PB, 0, g->stream>>>(g->kp, stencils, count, left, right);
+  }
+  CK(cudaGetLastError());
+  return MFC_OK;
+}
+
+mfc_status mfc_hllc_faces(mfc_grid* g, int dir, const double* wL, const double* wR, long long count, double* F, double* uf) {
+  if (!g || !wL || !wR || !F || !uf) return fail(MFC_ERR_ARG, "mfc_hllc_faces: NULL argument");
+  if (count < 0 || dir < 0 || dir >= g->ndim) return fail(MFC_ERR_ARG, "mfc_hllc_faces: bad count or direction");
+  if (mfc_status s = use_device(g)) return s;
+  if (count == 0) return MFC_OK;
+  CK(MFC_DISPATCH(g, (launch_hllc_unit<N, D>(g, dir, wL, wR, count, F, uf))));
   return MFC_OK;
 }
 

@@ -75,7 +75,8 @@ __device__ __forceinline__ bool prim_cell(const KP& kp, const double* q, double*
     const double rr = frcp(rho);
 #pragma unroll
     for (int d = 0; d < D; ++d) {
-      const double u = q[IM + d] * rr;
+      double u = q[IM + d] * rr;
+      u = fma(fma(-rho, u, q[IM + d]), rr, u);  // one residual step: the quotient to ~1/2 ulp (N2)
       w[IM + d] = u;
       usq = d == 0 ? u * u : fma(u, u, usq);
     }
@@ -144,7 +145,7 @@ __device__ __forceinline__ void weno5(double a, double b, double c, double d, do
 //   side K = L if (S_L >= 0 or S* >= 0) else R;  star = (K = L) ? !(S_L >= 0) : (S_R > 0).
 // With ds = S* - u_K (0 outside the fan), r = 1/(S_K - S*), chi - 1 = ds r, the star-state correction
 // S_K (q*_K - q_K) collapses to
-//   alpha_i rho_i, alpha_i, rho u_t :  q u_f,           u_f = u_K + S_K (chi - 1)
+//   alpha_i rho_i, alpha_i, rho u_t :  q u_f,           u_f = u_K + S_K (chi - 1) = chi S*
 //   rho u_n :  rho u_K^2 + p + S_K rho (chi ds + (chi-1) u_K)
 //   E       :  (E + p) u_K + S_K ((chi-1) E + chi ds rho S* + ds p r)        [uses chi/(S_K-u_K) = r]
 template <int N, int D, int DIR>
@@ -188,7 +189,8 @@ __device__ __forceinline__ bool hllc(const KP& kp, const double* wL, const doubl
   const double ds = star ? (Ss - unK) : 0.0;
   const double chim1 = ds * r;
   const double chi = 1.0 + chim1;
-  uf = fma(SK, chim1, unK);
+  // u_f = u_K + S_K (chi - 1) = chi S* inside the fan (no cancellation in this form), u_K outside
+  uf = star ? fma(chim1, Ss, Ss) : unK;
 #pragma unroll
   for (int i = 0; i < N; ++i) {
     F[i] = (useL ? wL[i] : wR[i]) * uf;

@@ -1,7 +1,16 @@
-"""The error measure of the parity bar (DESIGN.md §5): max-norm relative error per variable,
+"""The error measure of the parity bar (DESIGN.md §7): max-norm relative error per variable,
 each variable scaled by the largest magnitude within its GROUP (partial densities / momenta /
 energy / volume fractions).  Grouping the momentum components keeps a component that vanishes by
-symmetry (config 3's rho*v, every 1-D transverse direction) from being measured against round-off."""
+symmetry (config 3's rho*v, every 1-D transverse direction) from being measured against round-off.
+
+Rounding noise of the reference.  The fp64 oracle is itself only one rounding of its definition: it
+differs from the same text evaluated in 80-bit arithmetic (oracle_rhs_ld) by n64 = max|o64 - o80| per
+group.  Where the volume-fraction group of the reference is analytically zero — one fluid (alpha == 1), or
+uniform alpha wherever the fluid moves (configs 3 and 5 at t = 0: the bubble / droplet is at rest ahead of
+the shock) — d(alpha)/dt is the round-off of two cancelling terms of size |u|/dx, the whole reference IS
+rounding noise and a relative measure has no meaning.  Tests that pass `noise=` (they say why) allow 4*n64
+for the volume-fraction group only:  max|gpu - o64| <= tol*scale + 4*n64.  Every other group, and every
+test that does not pass `noise=`, is held to the bare relative bar."""
 import numpy as np
 
 
@@ -10,11 +19,18 @@ def groups(nfluids, ndim):
     return [list(range(0, N)), list(range(N, N + D)), [N + D], list(range(N + D + 1, 2 * N + D + 1))]
 
 
-def rel_err(a, ref, nfluids, ndim):
-    """max over variables of max|a-ref| / max_group|ref|; returns (worst, per-variable list)"""
+def group_noise(ref, ref_ld, nfluids, ndim):
+    """per-group max|o64 - o80|: the rounding noise of the fp64 reference"""
+    return [float(np.abs(ref[g] - ref_ld[g]).max()) for g in groups(nfluids, ndim)]
+
+
+def rel_err(a, ref, nfluids, ndim, noise=None):
+    """max over variables of max|a-ref| / max_group|ref| (volume-fraction group: (max|a-ref| - 4*noise)^+ if
+    noise is given); returns (worst, per-variable list)"""
     per = []
-    for g in groups(nfluids, ndim):
+    for gi, g in enumerate(groups(nfluids, ndim)):
         scale = max(float(np.abs(ref[g]).max()), 1e-300)
+        allow = 4.0 * noise[gi] if (noise is not None and gi == 3) else 0.0
         for v in g:
-            per.append(float(np.abs(a[v] - ref[v]).max()) / scale)
+            per.append(max(float(np.abs(a[v] - ref[v]).max()) - allow, 0.0) / scale)
     return max(per), per

@@ -8,7 +8,7 @@ import pytest
 
 import mfc_workloads as W
 from oracle import oracle as O
-from parity_norm import rel_err
+from parity_norm import group_noise, rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -35,6 +35,14 @@ def make_case(ndim, nfluids, n, bc, clamp=True, eps=1e-16):
     nn = tuple(n[d] if d < ndim else 1 for d in range(3))
     return W.Case("t", ndim, nn, tuple(0.7 / nn[d] if d < ndim else 1.0 for d in range(3)), nfluids,
                   gamma[:nfluids], pi_inf[:nfluids], (bc,) * 3, (bc,) * 3, weno_eps=eps, clamp=clamp)
+
+
+def oracle_rhs_with_noise(case, q, mask=7):
+    """fp64 oracle rhs and the per-group rounding noise of that reference (vs its 80-bit evaluation)"""
+    orc = O.Oracle(case)
+    ref = orc.rhs(q, dir_mask=mask)
+    assert orc.bad == 0
+    return ref, group_noise(ref, orc.rhs_ld(q, dir_mask=mask), case.nfluids, case.ndim)
 
 
 def gpu_rhs(torch, mfc, case, q, mask=7, seg=None):
@@ -78,16 +86,20 @@ ROUGH = [
 ]
 
 
+def rough_state(case, seed):
+    """cell-wise independent random state; alpha_lo=0.5 keeps WENO overshoots of alpha inside (0,1)"""
+    return W.random_admissible_state(case, seed=seed, alpha_lo=0.5)
+
+
 @pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_EXTRAP])
 @pytest.mark.parametrize("ndim,nfluids,n", ROUGH)
 def test_rhs_rough_state_all_directions(torch, mfc, ndim, nfluids, n, bc):
     case = make_case(ndim, nfluids, n, bc)
-    q = W.random_admissible_state(case, seed=5 + ndim)
-    orc = O.Oracle(case)
-    ref = orc.rhs(q)
-    assert orc.bad == 0
+    q = rough_state(case, 5 + ndim)
+    ref, noise = oracle_rhs_with_noise(case, q)
     got = gpu_rhs(torch, mfc, case, q)
-    worst, per = rel_err(got, ref, nfluids, ndim)
+    # one fluid: alpha == 1 and d(alpha)/dt is analytically zero — the volume-fraction group of the reference is rounding noise
+    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None)
     assert worst <= RHS_TOL, per
 
 
@@ -95,8 +107,10 @@ def test_rhs_rough_state_all_directions(torch, mfc, ndim, nfluids, n, bc):
                                                  (3, 2, (33, 18, 11), 2), (3, 2, (33, 18, 11), 4), (3, 3, (20, 9, 13), 5)])
 def test_rhs_single_directions(torch, mfc, ndim, nfluids, n, mask):
     case = make_case(ndim, nfluids, n, W.BC_EXTRAP)
-    q = W.random_admissible_state(case, seed=3)
-    ref = O.Oracle(case).rhs(q, dir_mask=mask)
+    q = rough_state(case, 3)
+    orc = O.Oracle(case)
+    ref = orc.rhs(q, dir_mask=mask)
+    assert orc.bad == 0
     got = gpu_rhs(torch, mfc, case, q, mask=mask)
     worst, per = rel_err(got, ref, nfluids, ndim)
     assert worst <= RHS_TOL, per
@@ -106,7 +120,7 @@ def test_rhs_single_directions(torch, mfc, ndim, nfluids, n, mask):
 def test_rhs_independent_of_segmentation(torch, mfc, seg):
     # segment boundaries only re-partition the work: each face flux sees the same inputs wherever they fall
     case = make_case(3, 2, (75, 21, 19), W.BC_PERIODIC)
-    q = W.random_admissible_state(case, seed=9)
+    q = rough_state(case, 9)
     ref = O.Oracle(case).rhs(q)
     base = gpu_rhs(torch, mfc, case, q)
     got = gpu_rhs(torch, mfc, case, q, seg=seg)
@@ -128,11 +142,12 @@ def test_rhs_uniform_state_is_exactly_zero(torch, mfc):
 def test_rhs_configs(torch, mfc, index, n):
     case = W.config(index, n=n)
     q = W.initial_state(case)
-    orc = O.Oracle(case)
-    ref = orc.rhs(q)
-    assert orc.bad == 0
+    ref, noise = oracle_rhs_with_noise(case, q)
     got = gpu_rhs(torch, mfc, case, q)
-    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    # configs 1, 3, 5 at t = 0: d(alpha)/dt is analytically zero (alpha == 1; alpha uniform wherever the
+    # fluid moves, the bubble / droplet being at rest ahead of the shock): the volume-fraction group is
+    # allowed the reference's own rounding noise (parity_norm).  configs 2 and 4 are held to the bare bar.
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim, None if index in (2, 4) else noise)
     assert worst <= RHS_TOL, per
 
 
@@ -148,9 +163,11 @@ def test_rhs_host_entry_point_matches_device_entry_point(torch, mfc):
 
 # ------------------------------------------------------------------ full-size parity (the bench launch configurations)
 def test_rhs_full_size_config4_elementwise(torch, mfc):
-    case = W.config(4)  # 256^3, the configuration bench.py times; the oracle needs ~20 s for it
+    case = W.config(4)  # 256^3, the configuration bench.py times; every cell, bare bar
     q = W.initial_state(case)
-    ref = O.Oracle(case).rhs(q)
+    orc = O.Oracle(case)
+    ref = orc.rhs(q)
+    assert orc.bad == 0
     got = gpu_rhs(torch, mfc, case, q)
     worst, per = rel_err(got, ref, case.nfluids, case.ndim)
     assert worst <= RHS_TOL, per
@@ -159,9 +176,9 @@ def test_rhs_full_size_config4_elementwise(torch, mfc):
 def test_rhs_full_size_config3_elementwise(torch, mfc):
     case = W.config(3)  # 1024^2 in full
     q = W.initial_state(case)
-    ref = O.Oracle(case).rhs(q)
+    ref, noise = oracle_rhs_with_noise(case, q)
     got = gpu_rhs(torch, mfc, case, q)
-    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim, noise)
     assert worst <= RHS_TOL, per
 
 
@@ -175,7 +192,7 @@ def _sampled_box_parity(torch, mfc, case, q, boxes, core):
     g.rhs(qd, rd)
     g.check()
     D = case.ndim
-    gots, refs = [], []
+    gots, refs, lds = [], [], []
     for lo3 in boxes:
         idx = []
         for d in range(3):
@@ -188,11 +205,13 @@ def _sampled_box_parity(torch, mfc, case, q, boxes, core):
                        (W.BC_EXTRAP,) * 3, weno_eps=case.weno_eps, clamp=case.clamp)
         ref = O.Oracle(scase).rhs(sub)
         refs.append(ref[:, 3:3 + core, 3:3 + core, 3:3 + core].reshape(case.neq, -1))
+        lds.append(O.Oracle(scase).rhs_ld(sub)[:, 3:3 + core, 3:3 + core, 3:3 + core].reshape(case.neq, -1))
         gi = [torch.as_tensor(idx[d][3:3 + core], device="cuda") for d in range(3)]
         got = rd.view(case.shape)[:, gi[2][:, None, None], gi[1][None, :, None], gi[0][None, None, :]]
         gots.append(got.cpu().numpy().reshape(case.neq, -1))
     g.close()
-    return rel_err(np.concatenate(gots, 1), np.concatenate(refs, 1), case.nfluids, case.ndim)
+    got, ref, ld = np.concatenate(gots, 1), np.concatenate(refs, 1), np.concatenate(lds, 1)
+    return rel_err(got, ref, case.nfluids, case.ndim, group_noise(ref, ld, case.nfluids, case.ndim))
 
 
 def test_rhs_full_size_config5_sampled(torch, mfc):
@@ -212,27 +231,50 @@ def test_rhs_full_size_config5_sampled(torch, mfc):
 
 
 # ------------------------------------------------------------------ RK3: stage arithmetic, clamp, 100 steps
-def test_rk3_single_step_with_clamp_firing(torch, mfc):
+def test_rk_stage_and_clamp_arithmetic_bit_exact(torch, mfc):
+    # dt = 0 removes L from every stage: what is left is the stage combination and the A10 clamp, which
+    # must reproduce the oracle bit for bit — including cells where the clamp fires.  The state is
+    # physically admissible (p > 0, rho > 0) but sits outside the clamp's bounds in a third of the cells.
     case = make_case(2, 3, (40, 17, 1), W.BC_PERIODIC, clamp=True)
-    q = W.random_admissible_state(case, seed=21)
-    N, D = 3, 2
+    sh = case.shape[1:]
     rng = np.random.default_rng(2)
-    # push volume fractions / partial densities out of bounds in a third of the cells
-    hit = rng.random(case.shape[1:]) < 0.33
-    q[N + D + 1][hit] = -1e-3
-    q[N + D + 2][hit] += 1e-3
-    q[0][rng.random(case.shape[1:]) < 0.05] *= 1e-9
-    orc = O.Oracle(case)
-    dt = 1e-7
+    a0 = np.where(rng.random(sh) < 0.33, 1e-9, rng.uniform(0.2, 0.4, sh))   # below the floor in a third of the cells
+    a1 = rng.uniform(0.2, 0.5, sh)
+    alpha = [a0, a1, 1.0 - a0 - a1 + np.where(rng.random(sh) < 0.2, 0.05, 0.0)]  # sum != 1 in places
+    arho = [np.where(rng.random(sh) < 0.1, -1e-12, a0 * 1.0), a1 * 1000.0, alpha[2] * 0.138]  # a slightly negative partial density
+    u = [rng.uniform(-10, 10, sh), rng.uniform(-10, 10, sh)]
+    q = np.ascontiguousarray(W.cons_from_prim(case, arho, u, rng.uniform(0.9e5, 1.1e5, sh), alpha))
     ref = q.copy()
-    orc.rk3_step(ref, dt)
+    orc = O.Oracle(case)
+    orc.rk3_step(ref, 0.0)
+    assert orc.bad == 0 and np.isfinite(ref).all() and not np.array_equal(ref, q)
     g = mfc.Grid.from_case(case)
     qd = torch.from_numpy(q).cuda()
-    g.rk3_step(qd, dt)
+    g.rk3_step(qd, 0.0)
+    g.check()
+    assert np.array_equal(qd.cpu().numpy(), ref)
+
+
+def test_rk3_step_with_clamp_firing_everywhere(torch, mfc):
+    # the water/air tube built with alpha = 1e-6 in the pure regions, run with a floor of 1e-5:
+    # the clamp fires in every cell after every stage
+    import dataclasses
+    case = dataclasses.replace(W.config(2, n=800), alpha_floor=1e-5)
+    q = W.initial_state(W.config(2, n=800))
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    for _ in range(20):
+        dt = orc.cfl_dt(ref, 0.5)
+        orc.rk3_step(ref, dt)
+        assert orc.bad == 0
+        g.rk3_step(qd, dt)
+    g.check()
     got = qd.cpu().numpy()
-    assert rel_err(got, ref, N, D)[0] <= 1e-13
-    a = got[N + D + 1:]
-    assert a.min() >= case.alpha_floor / (1 + 3 * case.alpha_floor) * (1 - 1e-15)
+    assert rel_err(got, ref, 2, 1)[0] <= STEP_TOL
+    a = got[4:]
+    assert a.min() >= 1e-5 / (1 + 2e-5) * (1 - 1e-15) and np.abs(a.sum(0) - 1).max() < 1e-4
 
 
 @pytest.mark.parametrize("index,n,nsteps", [(1, None, 100), (2, None, 100), (2, None, 500), (3, 128, 100), (4, 48, 50),

@@ -117,6 +117,38 @@ def test_weno_mirror_symmetry():
         assert l == pytest.approx(r2, rel=1e-12) and r == pytest.approx(l2, rel=1e-12)
 
 
+def test_weno_difference_form_is_the_textbook_form_and_rounds_to_half_an_ulp():
+    # Reading N2: the oracle evaluates f = c + sum_r omega_r (f^(r) - c) with the candidate
+    # deviations in first differences.  (i) It is the textbook sum_r omega_r f^(r) (Jiang-Shu
+    # candidates) for arbitrary data, up to the rounding of that textbook evaluation; (ii) on smooth data with an
+    # offset (a velocity field u0 + small variation) its fp64 result is within 1 ulp of the 80-bit evaluation —
+    # the property the parity bar needs, because the low-Mach HLLC flux amplifies velocity rounding by rho*c.
+    rng = np.random.default_rng(5)
+    worst_ulp = 0.0
+    for k in range(300):
+        if k < 150:
+            s = rng.normal(size=5) * 10 ** rng.uniform(-2, 2)
+            eps = 1e-6
+        else:
+            x0, h = rng.uniform(0, 6.28), 10 ** rng.uniform(-3, -1)
+            s = 10.0 + 3.0 * np.sin(x0 + h * np.arange(-2, 3))
+            eps = 1e-16
+        b = [13 / 12 * (s[0] - 2 * s[1] + s[2]) ** 2 + 0.25 * (s[0] - 4 * s[1] + 3 * s[2]) ** 2,
+             13 / 12 * (s[1] - 2 * s[2] + s[3]) ** 2 + 0.25 * (s[1] - s[3]) ** 2,
+             13 / 12 * (s[2] - 2 * s[3] + s[4]) ** 2 + 0.25 * (3 * s[2] - 4 * s[3] + s[4]) ** 2]
+        al = np.array([0.1, 0.6, 0.3]) / (np.array(b) + eps) ** 2
+        ar = np.array([0.3, 0.6, 0.1]) / (np.array(b) + eps) ** 2
+        pl = np.array([(2 * s[0] - 7 * s[1] + 11 * s[2]) / 6, (-s[1] + 5 * s[2] + 2 * s[3]) / 6, (2 * s[2] + 5 * s[3] - s[4]) / 6])
+        pr = np.array([(-s[0] + 5 * s[1] + 2 * s[2]) / 6, (2 * s[1] + 5 * s[2] - s[3]) / 6, (11 * s[2] - 7 * s[3] + 2 * s[4]) / 6])
+        l, r = O.weno5_js(s, eps)
+        scale = np.abs(s).max()
+        assert abs(l - (al / al.sum()) @ pl) <= 2e-14 * scale and abs(r - (ar / ar.sum()) @ pr) <= 2e-14 * scale
+        if k >= 150:
+            l80, r80 = O.weno5_js_ld(s, eps)
+            worst_ulp = max(worst_ulp, abs(l - l80) / np.spacing(abs(l80)), abs(r - r80) / np.spacing(abs(r80)))
+    assert worst_ulp <= 1.0, worst_ulp
+
+
 def test_weno_fifth_order_on_cell_averaged_sine():
     # brute-force refinement: error of the face value against the exact point value
     errs = []
