@@ -35,7 +35,7 @@ UNIT = "ns/cell/eqn/rhs_eval"
 # Algorithmic flops per cell per RHS evaluation of the plain definition (add/sub, mul, div, sqrt = 1 flop
 # each), counted by the operation-counting instantiation of the oracle and extrapolated to n -> infinity
 # (tests/test_host_logic.py re-derives them).  Key: BASELINE.json config index.
-ALG_FLOPS_PER_CELL_RHS = {1: 557.0, 2: 810.0, 3: 1872.0, 4: 3186.0, 5: 3945.0}
+ALG_FLOPS_PER_CELL_RHS = {1: 538.0, 2: 779.0, 3: 1798.0, 4: 3057.0, 5: 3780.0}
 # FP64 peak "derived from unit counts and clocks": 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz.
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 # DFMA-chain microbenchmark on this pool's B200: 17.05e12 DFMA/s = 34.1 TFLOP/s (SM clock ~1.80 GHz under FP64 load)
