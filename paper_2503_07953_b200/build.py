@@ -9,7 +9,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
-LIB = os.path.join(HERE, "libmfc_b200.so")
+# MFC_B200_LIB names another library file to build/load (tuning variants); MFC_B200_NVCC_EXTRA adds nvcc flags.
+LIB = os.environ.get("MFC_B200_LIB") or os.path.join(HERE, "libmfc_b200.so")
 SRC = [os.path.join(HERE, "csrc", "mfc_b200.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "mfc_device.cuh"), os.path.join(ROOT, "include", "mfc_b200.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -20,7 +21,8 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
         return LIB
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
+    extra = os.environ.get("MFC_B200_NVCC_EXTRA", "").split()
+    cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
     subprocess.check_call(cmd)
     return LIB
 

@@ -24,8 +24,21 @@
 namespace mfc {
 
 constexpr unsigned FULL = 0xffffffffu;
-constexpr int XW = 4;     // warps per block, sweep_x
-constexpr int MB = 128;   // threads per block, sweep_march
+// Tuning knobs (compile-time; the defaults are the measured best on B200).
+#ifndef MFC_XW
+#define MFC_XW 4          // warps per block, sweep_x
+#endif
+#ifndef MFC_XMINB
+#define MFC_XMINB 1       // __launch_bounds__ min blocks per SM, sweep_x
+#endif
+#ifndef MFC_MB
+#define MFC_MB 128        // threads per block, sweep_march
+#endif
+#ifndef MFC_MMINB
+#define MFC_MMINB 1       // __launch_bounds__ min blocks per SM, sweep_march
+#endif
+constexpr int XW = MFC_XW;
+constexpr int MB = MFC_MB;
 constexpr int PB = 256;   // threads per block, pointwise kernels
 
 // ------------------------------------------------------------------------------------------------ prim
@@ -49,7 +62,7 @@ __global__ void __launch_bounds__(PB) prim_kernel(const __grid_constant__ KP kp,
 // Lane with position p: reconstructs cell i (both values), solves face i-1/2 (p >= 1) with the left
 // state of lane p-1, and updates cell i-1 (p >= 2) with the flux of lane p-1.
 template <int N, int D, bool ACCUM>
-__global__ void __launch_bounds__(XW * 32) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
+__global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                    double* __restrict__ rhs, int seglen, int nseg) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
   __shared__ double ring[XW][NEQ][64];
@@ -157,7 +170,7 @@ __global__ void __launch_bounds__(XW * 32) sweep_x(const __grid_constant__ KP kp
 // ring slot (sl+k)%5 holds the primitives of cell g-2+k.  The cell g+3 is prefetched as conservatives
 // into registers during the step and converted at the start of the next one.
 template <int N, int D, int DIR, bool ACCUM>
-__global__ void __launch_bounds__(MB) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
+__global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                   double* __restrict__ rhs, int seglen, int nseg) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
   extern __shared__ double ring[];  // [5][NEQ][MB]
@@ -608,6 +621,15 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
   return cudaGetLastError();
 }
 
+#ifdef MFC_ONLY_23  // tuning builds: one instantiation only
+#define MFC_DISPATCH(g, EXPR)                                  \
+  [&]() -> cudaError_t {                                       \
+    switch ((g)->nf * 10 + (g)->ndim) {                        \
+      case 23: { constexpr int N = 2, D = 3; return EXPR; }    \
+    }                                                          \
+    return cudaErrorInvalidValue;                              \
+  }()
+#else
 #define MFC_DISPATCH(g, EXPR)                                  \
   [&]() -> cudaError_t {                                       \
     switch ((g)->nf * 10 + (g)->ndim) {                        \
@@ -623,6 +645,7 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
     }                                                          \
     return cudaErrorInvalidValue;                              \
   }()
+#endif
 
 static mfc_status use_device(const mfc_grid* g) {
   CK(cudaSetDevice(g->device));
