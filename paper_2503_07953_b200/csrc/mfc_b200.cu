@@ -8,7 +8,7 @@
 //   sweep_march     y/z-direction: lanes span x (coalesced), each thread marches along the sweep
 //                   direction with a thread-private 5-cell ring of primitives in shared memory; the
 //                   previous face's left state and flux stay in registers (O1-O5)
-//   rk_kernel       SSP-RK3 stage combination + A10 clamp (O6)
+//   rk_cell         SSP-RK3 stage combination + A10 clamp (O6), applied by the last sweep of each stage
 //   cfl_kernel      max_cells sum_d (|u_d|+c)/dx_d by warp shuffles + block reduce + integer atomicMax (O7)
 // No face state, flux or primitive array is ever written to HBM; ghost cells are index maps (O1).
 #include "../../include/mfc_b200.h"
@@ -56,14 +56,57 @@ __global__ void __launch_bounds__(PB) prim_kernel(const __grid_constant__ KP kp,
   for (int v = 0; v < NEQ; ++v) w[v * kp.ncells + c] = wc[v];
 }
 
+// ------------------------------------------------------------------------------------------------ RK stage of one cell
+// O6 (PAPER.md:207-211), each product and sum rounded individually in the printed grouping:
+//   stage 1: q1 = q + dt L        stage 2: q2 = 3/4 q + 1/4 (q1 + dt L)        stage 3: q = 1/3 q + 2/3 (q2 + dt L)
+// followed by the A10 clamp of the new stage state.  r holds L on entry and the new stage state on exit;
+// qn = the cell of q^n, qs = the cell of the stage state the RHS was evaluated on (unused in stage 1).
+template <int N, int D, int STAGE>
+__device__ __forceinline__ void rk_cell(const KP& kp, double dt, const double* qn, const double* qs, double* r) {
+  constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) {
+    const double dl = __dmul_rn(dt, r[v]);
+    if (STAGE == 1) {
+      r[v] = __dadd_rn(qn[v], dl);
+    } else if (STAGE == 2) {
+      r[v] = __dadd_rn(__dmul_rn(0.75, qn[v]), __dmul_rn(0.25, __dadd_rn(qs[v], dl)));
+    } else {
+      r[v] = __dadd_rn(__dmul_rn(1.0 / 3.0, qn[v]), __dmul_rn(2.0 / 3.0, __dadd_rn(qs[v], dl)));
+    }
+  }
+  if (kp.clamp) {  // A10
+#pragma unroll
+    for (int i = 0; i < N; ++i) r[i] = r[i] < 0.0 ? 0.0 : r[i];
+    bool marked = false;
+#pragma unroll
+    for (int i = 0; i < N; ++i)
+      if (r[IA + i] < kp.alpha_floor) {
+        r[IA + i] = kp.alpha_floor;
+        marked = true;
+      }
+    if (marked) {
+      double sum = r[IA];
+#pragma unroll
+      for (int i = 1; i < N; ++i) sum = __dadd_rn(sum, r[IA + i]);
+#pragma unroll
+      for (int i = 0; i < N; ++i) r[IA + i] = __ddiv_rn(r[IA + i], sum);
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ x sweep
 // Positions along a segment [s0, s0+L): load position pos <-> cell s0-3+pos (pos = 0..L+5);
 // reconstruction position p <-> cell i = s0-1+p (p = 0..L+1), whose stencil sits at load positions p..p+4.
 // Lane with position p: reconstructs cell i (both values), solves face i-1/2 (p >= 1) with the left
 // state of lane p-1, and updates cell i-1 (p >= 2) with the flux of lane p-1.
-template <int N, int D, bool ACCUM>
+// STAGE = 0: rhs = (or +=) the x part of L(q).  STAGE = 1..3 (the last sweep of an RK stage): the
+// finished L of the cell goes straight through rk_cell and the new stage state is written instead of L —
+// stages 1 and 2 in place over the partial L in `rhs`, stage 3 over q^n in `qnn` (each cell of those buffers is
+// read and written by its one thread only; `q`, the state being swept, is never written).
+template <int N, int D, bool ACCUM, int STAGE>
 __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
-                                                   double* __restrict__ rhs, int seglen, int nseg) {
+                                                   double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
   __shared__ double ring[XW][NEQ][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -150,12 +193,33 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
     if (p >= 2 && p < nrec) {  // cell i-1 = s0 + p - 2: eq.(10) and the alpha_i div(u) source
       const int i = s0 + p - 2;
       const double du = (uf - ufm) * idx;
+      if (STAGE == 0) {
 #pragma unroll
-      for (int v = 0; v < NEQ; ++v) {
-        double r = (Fm[v] - F[v]) * idx;
-        if (v >= IA) r = fma(rg[v][(p + 1) & 63], du, r);
-        if (ACCUM) r += rrow[v * kp.ncells + i];
-        rrow[v * kp.ncells + i] = r;
+        for (int v = 0; v < NEQ; ++v) {
+          double r = (Fm[v] - F[v]) * idx;
+          if (v >= IA) r = fma(rg[v][(p + 1) & 63], du, r);
+          if (ACCUM) r += rrow[v * kp.ncells + i];
+          rrow[v * kp.ncells + i] = r;
+        }
+      } else {
+        double r[NEQ];
+#pragma unroll
+        for (int v = 0; v < NEQ; ++v) {
+          r[v] = (Fm[v] - F[v]) * idx;
+          if (v >= IA) r[v] = fma(rg[v][(p + 1) & 63], du, r[v]);
+          if (ACCUM) r[v] += rrow[v * kp.ncells + i];
+        }
+        const long long off = row * nx + i;
+        double qnc[NEQ], qsc[NEQ];
+#pragma unroll
+        for (int v = 0; v < NEQ; ++v) {
+          qnc[v] = qnn[v * kp.ncells + off];
+          qsc[v] = STAGE >= 2 ? __ldg(q + v * kp.ncells + off) : 0.0;
+        }
+        rk_cell<N, D, STAGE>(kp, dt, qnc, qsc, r);
+        double* out = STAGE == 3 ? qnn : rhs;
+#pragma unroll
+        for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + off] = r[v];
       }
     }
     __syncwarp();
@@ -169,11 +233,25 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
 // Thread <-> (column, segment [s0, s0+L) along DIR).  Step p = 0..L+1 handles cell g = s0-1+p:
 // ring slot (sl+k)%5 holds the primitives of cell g-2+k.  The cell g+3 is prefetched as conservatives
 // into registers during the step and converted at the start of the next one.
-template <int N, int D, int DIR, bool ACCUM>
+// STAGE as in sweep_x.  The operands of the cell update of step p (its partial L, and for STAGE >= 1 its q^n and
+// stage-state cells) are fetched by cp.async into thread-private shared-memory slots at the top of the step and
+// waited for just before the update, so their latency hides behind the step's arithmetic without holding registers.
+__device__ __forceinline__ void cp_async8(double* sdst, const double* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(sdst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__host__ __device__ constexpr int march_slots(bool accum, int stage) {
+  return 5 + (accum ? 1 : 0) + (stage >= 1 ? 1 : 0) + (stage >= 2 ? 1 : 0);
+}
+
+template <int N, int D, int DIR, bool ACCUM, int STAGE>
 __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
-                                                  double* __restrict__ rhs, int seglen, int nseg) {
+                                                  double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
-  extern __shared__ double ring[];  // [5][NEQ][MB]
+  constexpr int S_ACC = 5, S_QN = 5 + (ACCUM ? 1 : 0), S_QS = S_QN + 1;
+  extern __shared__ double ring[];  // [march_slots(ACCUM, STAGE)][NEQ][MB]
   const int n = kp.n[DIR];
   const long long ncols = kp.ncells / n;
   const long long id = (long long)blockIdx.x * MB + threadIdx.x;
@@ -230,10 +308,14 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
     convert(s4);
     if (p <= L) loadq(s0 + 2 + p);
     const long long offc = base + (long long)(s0 + p - 2) * stride;  // cell g-1 (valid for p >= 2)
-    double racc[NEQ];
-    if (ACCUM && p >= 2) {
+    if ((ACCUM || STAGE >= 1) && p >= 2) {
 #pragma unroll
-      for (int v = 0; v < NEQ; ++v) racc[v] = rhs[v * kp.ncells + offc];
+      for (int v = 0; v < NEQ; ++v) {
+        if (ACCUM) cp_async8(&RG(S_ACC, v), rhs + v * kp.ncells + offc);
+        if (STAGE >= 1) cp_async8(&RG(S_QN, v), qnn + v * kp.ncells + offc);
+        if (STAGE >= 2) cp_async8(&RG(S_QS, v), q + v * kp.ncells + offc);
+      }
+      cp_async_commit();
     }
     double WL[NEQ], WR[NEQ];
 #pragma unroll
@@ -244,13 +326,29 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
       bad |= hllc<N, D, DIR>(kp, WLp, WR, F, uf);
       if (p >= 2) {
         const double du = (uf - ufp) * idx;
+        double r[NEQ];
 #pragma unroll
         for (int v = 0; v < NEQ; ++v) {
-          double r = (Fp[v] - F[v]) * idx;
-          if (v >= IA) r = fma(RG(s1, v), du, r);
-          if (ACCUM) r += racc[v];
-          rhs[v * kp.ncells + offc] = r;
+          r[v] = (Fp[v] - F[v]) * idx;
+          if (v >= IA) r[v] = fma(RG(s1, v), du, r[v]);
         }
+        if (ACCUM || STAGE >= 1) cp_async_wait_all();
+        if (ACCUM) {
+#pragma unroll
+          for (int v = 0; v < NEQ; ++v) r[v] += RG(S_ACC, v);
+        }
+        if (STAGE >= 1) {
+          double qnc[NEQ], qsc[NEQ];
+#pragma unroll
+          for (int v = 0; v < NEQ; ++v) {
+            qnc[v] = RG(S_QN, v);
+            qsc[v] = STAGE >= 2 ? RG(S_QS, v) : 0.0;
+          }
+          rk_cell<N, D, STAGE>(kp, dt, qnc, qsc, r);
+        }
+        double* out = STAGE == 3 ? qnn : rhs;
+#pragma unroll
+        for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + offc] = r[v];
       }
 #pragma unroll
       for (int v = 0; v < NEQ; ++v) Fp[v] = F[v];
@@ -262,51 +360,6 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
   }
 #undef RG
   if (bad) *kp.flag = 1;
-}
-
-// ------------------------------------------------------------------------------------------------ RK stage
-// O6 (PAPER.md:207-211), each product and sum rounded individually in the printed grouping:
-//   stage 1: q1 = q + dt L        stage 2: q1 = 3/4 q + 1/4 (q1 + dt L)        stage 3: q = 1/3 q + 2/3 (q1 + dt L)
-// followed by the A10 clamp of the new stage state.  `out` may alias `q` or `q1` (cell-local).
-template <int N, int D, int STAGE>
-__global__ void __launch_bounds__(PB) rk_kernel(const __grid_constant__ KP kp, const double* q, const double* q1,
-                                                const double* __restrict__ Lq, double* out, double dt) {
-  constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
-  const long long c = (long long)blockIdx.x * PB + threadIdx.x;
-  if (c >= kp.ncells) return;
-  double r[NEQ];
-#pragma unroll
-  for (int v = 0; v < NEQ; ++v) {
-    const long long t = v * kp.ncells + c;
-    const double dl = __dmul_rn(dt, Lq[t]);
-    if (STAGE == 1) {
-      r[v] = __dadd_rn(q[t], dl);
-    } else if (STAGE == 2) {
-      r[v] = __dadd_rn(__dmul_rn(0.75, q[t]), __dmul_rn(0.25, __dadd_rn(q1[t], dl)));
-    } else {
-      r[v] = __dadd_rn(__dmul_rn(1.0 / 3.0, q[t]), __dmul_rn(2.0 / 3.0, __dadd_rn(q1[t], dl)));
-    }
-  }
-  if (kp.clamp) {  // A10
-#pragma unroll
-    for (int i = 0; i < N; ++i) r[i] = r[i] < 0.0 ? 0.0 : r[i];
-    bool marked = false;
-#pragma unroll
-    for (int i = 0; i < N; ++i)
-      if (r[IA + i] < kp.alpha_floor) {
-        r[IA + i] = kp.alpha_floor;
-        marked = true;
-      }
-    if (marked) {
-      double s = r[IA];
-#pragma unroll
-      for (int i = 1; i < N; ++i) s = __dadd_rn(s, r[IA + i]);
-#pragma unroll
-      for (int i = 0; i < N; ++i) r[IA + i] = __ddiv_rn(r[IA + i], s);
-    }
-  }
-#pragma unroll
-  for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + c] = r[v];
 }
 
 // ------------------------------------------------------------------------------------------------ CFL
@@ -519,8 +572,8 @@ static cudaError_t launch_prim(mfc_grid* g, const double* q, double* w) {
   return cudaGetLastError();
 }
 
-template <int N, int D, int DIR, bool ACCUM>
-static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs) {
+template <int N, int D, int DIR, bool ACCUM, int STAGE>
+static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, double* qn, double dt) {
   if constexpr (DIR < D) {
     constexpr int NEQ = 2 * N + D + 1;
     const int n = g->kp.n[DIR];
@@ -528,8 +581,8 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs) {
     const int nseg = (n + seglen - 1) / seglen;
     const long long threads = g->kp.ncells / n * nseg;
     const long long nb = (threads + MB - 1) / MB;
-    const size_t smem = sizeof(double) * 5 * NEQ * MB;
-    auto kern = sweep_march<N, D, DIR, ACCUM>;
+    const size_t smem = sizeof(double) * march_slots(ACCUM, STAGE) * NEQ * MB;
+    auto kern = sweep_march<N, D, DIR, ACCUM, STAGE>;
     static bool attr_done[16] = {};
     if (!attr_done[g->device & 15]) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -537,22 +590,22 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs) {
       attr_done[g->device & 15] = true;
     }
     Scope sc(g, DIR == 1 ? MFC_K_SWEEP_Y : MFC_K_SWEEP_Z);
-    kern<<<(unsigned)nb, MB, smem, g->stream>>>(g->kp, q, rhs, seglen, nseg);
+    kern<<<(unsigned)nb, MB, smem, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt);
     return cudaGetLastError();
   } else {
     return cudaSuccess;
   }
 }
 
-template <int N, int D, bool ACCUM>
-static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs) {
+template <int N, int D, bool ACCUM, int STAGE>
+static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* qn, double dt) {
   const int nx = g->kp.n[0];
   const int seglen = g->seg[0];
   const int nseg = (nx + seglen - 1) / seglen;
   const long long warps = g->kp.ncells / nx * nseg;
   const long long nb = (warps + XW - 1) / XW;
   Scope sc(g, MFC_K_SWEEP_X);
-  sweep_x<N, D, ACCUM><<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg);
+  sweep_x<N, D, ACCUM, STAGE><<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt);
   return cudaGetLastError();
 }
 
@@ -562,40 +615,47 @@ static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mas
   const int all = (1 << D) - 1;
   cudaError_t e;
   if ((mask & all) == all) {
-    if ((e = launch_x<N, D, false>(g, q, rhs)) != cudaSuccess) return e;
+    if ((e = launch_x<N, D, false, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   } else {
     if ((e = cudaMemsetAsync(rhs, 0, state_bytes(g), g->stream)) != cudaSuccess) return e;
     if (mask & 1)
-      if ((e = launch_x<N, D, true>(g, q, rhs)) != cudaSuccess) return e;
+      if ((e = launch_x<N, D, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   }
   if (D >= 2 && (mask & 2))
-    if ((e = launch_march<N, D, 1, true>(g, q, rhs)) != cudaSuccess) return e;
+    if ((e = launch_march<N, D, 1, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   if (D >= 3 && (mask & 4))
-    if ((e = launch_march<N, D, 2, true>(g, q, rhs)) != cudaSuccess) return e;
+    if ((e = launch_march<N, D, 2, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   return cudaSuccess;
 }
 
+// One RK stage: L(qs) by the D sweeps, the last of which applies the stage combination and the clamp itself
+// (no separate RK kernel, the finished L never goes to HBM).  Stages 1 and 2 leave the new stage state in `work`
+// (where the partial L was), stage 3 writes q^{n+1} over q^n.
+template <int N, int D, int STAGE>
+static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, double* qn, double dt) {
+  cudaError_t e;
+  if constexpr (D == 1) {
+    return launch_x<N, D, false, STAGE>(g, qs, work, qn, dt);
+  } else {
+    if ((e = launch_x<N, D, false, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
+    if constexpr (D == 2) {
+      return launch_march<N, D, 1, true, STAGE>(g, qs, work, qn, dt);
+    } else {
+      if ((e = launch_march<N, D, 1, true, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
+      return launch_march<N, D, 2, true, STAGE>(g, qs, work, qn, dt);
+    }
+  }
+}
+
+// O6: q^n in `q` (caller's), two work arrays A = Lq, B = q1:
+//   stage 1 sweeps q,  partial L in A, q1 ends in A;   stage 2 sweeps A, partial L in B, q2 ends in B;
+//   stage 3 sweeps B,  partial L in A, q^{n+1} ends in q.
 template <int N, int D>
 static cudaError_t launch_rk3(mfc_grid* g, double* q, double dt) {
-  const long long nb = (g->kp.ncells + PB - 1) / PB;
-  const int all = (1 << D) - 1;
   cudaError_t e;
-  if ((e = launch_rhs<N, D>(g, q, g->Lq, all)) != cudaSuccess) return e;
-  {
-    Scope sc(g, MFC_K_RK);
-    rk_kernel<N, D, 1><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->q1, g->Lq, g->q1, dt);
-  }
-  if ((e = launch_rhs<N, D>(g, g->q1, g->Lq, all)) != cudaSuccess) return e;
-  {
-    Scope sc(g, MFC_K_RK);
-    rk_kernel<N, D, 2><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->q1, g->Lq, g->q1, dt);
-  }
-  if ((e = launch_rhs<N, D>(g, g->q1, g->Lq, all)) != cudaSuccess) return e;
-  {
-    Scope sc(g, MFC_K_RK);
-    rk_kernel<N, D, 3><<<(unsigned)nb, PB, 0, g->stream>>>(g->kp, q, g->q1, g->Lq, q, dt);
-  }
-  return cudaGetLastError();
+  if ((e = launch_stage<N, D, 1>(g, q, g->Lq, q, dt)) != cudaSuccess) return e;
+  if ((e = launch_stage<N, D, 2>(g, g->Lq, g->q1, q, dt)) != cudaSuccess) return e;
+  return launch_stage<N, D, 3>(g, g->q1, g->Lq, q, dt);
 }
 
 template <int N, int D>
