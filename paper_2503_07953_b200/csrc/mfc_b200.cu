@@ -37,7 +37,11 @@ constexpr unsigned FULL = 0xffffffffu;
 #ifndef MFC_MMINB
 #define MFC_MMINB 1       // __launch_bounds__ min blocks per SM, sweep_march
 #endif
+#ifndef MFC_MUNROLL
+#define MFC_MUNROLL 1    // unroll factor of the marching loop, sweep_march
+#endif
 constexpr int XW = MFC_XW;
+constexpr int MUNROLL = MFC_MUNROLL;
 constexpr int MB = MFC_MB;
 constexpr int PB = 256;   // threads per block, pointwise kernels
 
@@ -230,9 +234,11 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
 }
 
 // ------------------------------------------------------------------------------------------------ y/z sweep
-// Thread <-> (column, segment [s0, s0+L) along DIR).  Step p = 0..L+1 handles cell g = s0-1+p:
-// ring slot (sl+k)%5 holds the primitives of cell g-2+k.  The cell g+3 is prefetched as conservatives
-// into registers during the step and converted at the start of the next one.
+// Thread <-> (column, segment [s0, s0+L) along DIR).  Step p = 0..L+1 handles cell g = s0-1+p, whose stencil is
+// cells g-2..g+2.  What WENO needs of a cell is formed ONCE, when the cell enters the stencil as cell g+2, and
+// carried in thread-private shared-memory rings: its primitives w (3 slots: g-1, g, g+1), its first
+// difference d = w - w_prev (3 slots: d1, d2, d3) and u = 13/3 (d - d_prev)^2 + 4 eps (2 slots: u0, u1).  The
+// entering cell (g+2) was prefetched as conservatives into registers during the previous step.
 // STAGE as in sweep_x.  The operands of the cell update of step p (its partial L, and for STAGE >= 1 its q^n and
 // stage-state cells) are fetched by cp.async into thread-private shared-memory slots at the top of the step and
 // waited for just before the update, so their latency hides behind the step's arithmetic without holding registers.
@@ -242,121 +248,218 @@ __device__ __forceinline__ void cp_async8(double* sdst, const double* gsrc) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+constexpr int MARCH_RING = 8;  // 3 w + 3 d + 2 u slots
 __host__ __device__ constexpr int march_slots(bool accum, int stage) {
-  return 5 + (accum ? 1 : 0) + (stage >= 1 ? 1 : 0) + (stage >= 2 ? 1 : 0);
+  return MARCH_RING + (accum ? 1 : 0) + (stage >= 1 ? 1 : 0) + (stage >= 2 ? 1 : 0);
 }
 
 template <int N, int D, int DIR, bool ACCUM, int STAGE>
 __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                   double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
-  constexpr int S_ACC = 5, S_QN = 5 + (ACCUM ? 1 : 0), S_QS = S_QN + 1;
-  extern __shared__ double ring[];  // [march_slots(ACCUM, STAGE)][NEQ][MB]
+  constexpr int NH = (NEQ + 1) / 2;  // variables are stored in pairs (double2) so that every ring access moves two
+  constexpr int SLOT = NH * MB;      // double2 per slot
+  constexpr int S_D = 3, S_U = 6, S_ACC = MARCH_RING, S_QN = MARCH_RING + (ACCUM ? 1 : 0), S_QS = S_QN + 1;
+  extern __shared__ double2 ring[];  // PAIR: [slots][NH][MB] double2 = variables (2h, 2h+1); else [slots][2 NH][MB] doubles
   const int n = kp.n[DIR];
-  const long long ncols = kp.ncells / n;
+  const int ncols = (int)(kp.ncells / n);
   const long long id = (long long)blockIdx.x * MB + threadIdx.x;
-  if (id >= ncols * nseg) return;
+  if (id >= (long long)ncols * nseg) return;
   const int seg = (int)(id / ncols);
-  const long long col = id % ncols;
-  long long base, stride;
+  const int col = (int)(id - (long long)seg * ncols);
+  // cell offsets within one variable fit 32 bits (mfc_init_grid refuses grids of 2^31 cells or more)
+  int base, stride;
   if (DIR == 1) {
     const int nx = kp.n[0];
-    const long long k = col / nx;
-    base = k * nx * (long long)kp.n[1] + (col - k * nx);
+    const int k = col / nx;
+    base = k * nx * kp.n[1] + (col - k * nx);
     stride = nx;
   } else {
     base = col;
-    stride = (long long)kp.n[0] * kp.n[1];
+    stride = kp.n[0] * kp.n[1];
   }
   const int s0 = seg * seglen;
   const int L = min(seglen, n - s0);
   const int lo = kp.bc_lo[DIR], hi = kp.bc_hi[DIR];
   const double idx = kp.inv_dx[DIR];
-  double* R = ring + threadIdx.x;
-#define RG(slot, v) R[((slot) * NEQ + (v)) * MB]
+#ifndef MFC_PAIR
+#define MFC_PAIR 1
+#endif
+  constexpr bool PAIR = MFC_PAIR != 0;
+  // BF: the prefetch and the cp.async staging are issued unconditionally (on a valid, unused cell outside their range)
+  // instead of under a branch.  Measured on B200: 2 % faster for z, 3.5 % slower for y.
+#ifndef MFC_BF
+#define MFC_BF (DIR == 2)
+#endif
+  constexpr bool BF = MFC_BF;
+  // element (double2 offset o within the ring, pair h): one 16-byte access (PAIR) or two 8-byte accesses
+  auto ld2 = [&](int o, int h) -> double2 {
+    if (PAIR) return ring[o + h * MB + threadIdx.x];
+    const double* b = reinterpret_cast<const double*>(ring) + 2 * o + 2 * h * MB + threadIdx.x;
+    return make_double2(b[0], b[MB]);
+  };
+  auto st2 = [&](int o, int h, double2 x) {
+    if (PAIR) {
+      ring[o + h * MB + threadIdx.x] = x;
+    } else {
+      double* b = reinterpret_cast<double*>(ring) + 2 * o + 2 * h * MB + threadIdx.x;
+      b[0] = x.x;
+      b[MB] = x.y;
+    }
+  };
+  auto elem = [&](int o, int v) -> double* {  // address of variable v in the slot at double2 offset o
+    double* b = reinterpret_cast<double*>(ring);
+    return PAIR ? b + 2 * (o + (v / 2) * MB + threadIdx.x) + (v & 1) : b + 2 * o + v * MB + threadIdx.x;
+  };
+#define RG(slot, v) (*elem((slot) * SLOT, (v)))
   bool bad = false;
   double qn[NEQ];
-  auto loadq = [&](int cell) {
-    const long long off = base + (long long)ghost_index(cell, n, lo, hi) * stride;
+  auto loadq = [&](int off) {
 #pragma unroll
     for (int v = 0; v < NEQ; ++v) qn[v] = __ldg(q + v * kp.ncells + off);
   };
-  auto convert = [&](int slot) {
-    double w[NEQ];
-    bad |= prim_cell<N, D, false>(kp, qn, w);
+  // rotating slot offsets (in doubles): i0 = oldest of the 3-slot rings (w of cell g-1, d1), i2 = newest;
+  // j0 = older of the 2 u slots.
+  int i0 = 0, i1 = SLOT, i2 = 2 * SLOT, j0 = 0, j1 = SLOT;
+  {  // prologue: cells s0-3 .. s0 enter one by one (the first differences of the first two are never used)
+    double wp[NEQ], dp[NEQ];
 #pragma unroll
-    for (int v = 0; v < NEQ; ++v) RG(slot, v) = w[v];
-  };
+    for (int v = 0; v < NEQ; ++v) wp[v] = dp[v] = 0.0;
 #pragma unroll 1
-  for (int m = 0; m < 4; ++m) {
-    loadq(s0 - 3 + m);
-    convert(m);
+    for (int m = 0; m < 4; ++m) {
+      loadq(base + ghost_index(s0 - 3 + m, n, lo, hi) * stride);
+      double w[NEQ];
+      bad |= prim_cell<N, D, false>(kp, qn, w);
+      double dn[2 * NH], un[2 * NH], wn[2 * NH];
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) {
+        const double d = w[v] - wp[v];
+        wn[v] = w[v];
+        dn[v] = d;
+        un[v] = weno5_u(d - dp[v], kp.eps4);
+        wp[v] = w[v];
+        dp[v] = d;
+      }
+      if (NEQ & 1) wn[NEQ] = dn[NEQ] = un[NEQ] = 0.0;
+#pragma unroll
+      for (int h = 0; h < NH; ++h) {
+        st2(i0, h, make_double2(wn[2 * h], wn[2 * h + 1]));
+        st2(S_D * SLOT + i0, h, make_double2(dn[2 * h], dn[2 * h + 1]));
+        st2(S_U * SLOT + j0, h, make_double2(un[2 * h], un[2 * h + 1]));
+      }
+      const int t = i0;
+      i0 = i1, i1 = i2, i2 = t;
+      const int u = j0;
+      j0 = j1, j1 = u;
+    }
   }
-  loadq(s0 + 1);
+  loadq(base + ghost_index(s0 + 1, n, lo, hi) * stride);
+  // In the loop the cell to prefetch, s0+2+p, is never below 0, so its ghost map (O1) is: itself below n, else
+  // (periodic) itself minus n, reduced once or twice more when n < 3, or (extrapolation) n-1.  Offsets advance
+  // by one stride per step.
+  int cl = s0 + 2;                          // logical cell to prefetch during step p
+  const int nwrap = hi == BC_PERIODIC ? n : 0x7fffffff;  // period of the ghost map at the high end (none: extrapolation clamps)
 
   double WLp[NEQ], Fp[NEQ], ufp = 0.0;
 #pragma unroll
   for (int v = 0; v < NEQ; ++v) WLp[v] = Fp[v] = 0.0;
-  int sl = 0;
-#pragma unroll 1
+  int offc = base + (s0 - 2) * stride;      // cell g-1 of step p (used for p >= 2)
+#pragma unroll(MUNROLL)
   for (int p = 0; p <= L + 1; ++p) {
-    int s1 = sl + 1, s2 = sl + 2, s3 = sl + 3, s4 = sl + 4;
-    s1 -= s1 >= 5 ? 5 : 0;
-    s2 -= s2 >= 5 ? 5 : 0;
-    s3 -= s3 >= 5 ? 5 : 0;
-    s4 -= s4 >= 5 ? 5 : 0;
-    convert(s4);
-    if (p <= L) loadq(s0 + 2 + p);
-    const long long offc = base + (long long)(s0 + p - 2) * stride;  // cell g-1 (valid for p >= 2)
-    if ((ACCUM || STAGE >= 1) && p >= 2) {
+    double am[N];  // alpha_i of cell g-1 (source term of its update), read before its slot is reused
+#pragma unroll
+    for (int i = 0; i < N; ++i) am[i] = *elem(i0, IA + i);
+    double w[NEQ];
+    bad |= prim_cell<N, D, false>(kp, qn, w);  // cell g+2
+    {  // prefetch of cell s0+3+p, branch-free (in the last step, p = L+1, the value is not used; any valid cell will do)
+      int gl = cl;
+      gl -= gl >= nwrap ? nwrap : 0;
+      gl -= gl >= nwrap ? nwrap : 0;
+      gl -= gl >= nwrap ? nwrap : 0;
+      gl = min(gl, n - 1);
+      if (BF || p <= L) loadq(base + gl * stride);
+    }
+    ++cl;
+    if ((ACCUM || STAGE >= 1) && (BF || p >= 2)) {  // operands of this step's update (BF, p < 2: a valid cell, unused)
+      const int offs = p >= 2 ? offc : base;
 #pragma unroll
       for (int v = 0; v < NEQ; ++v) {
-        if (ACCUM) cp_async8(&RG(S_ACC, v), rhs + v * kp.ncells + offc);
-        if (STAGE >= 1) cp_async8(&RG(S_QN, v), qnn + v * kp.ncells + offc);
-        if (STAGE >= 2) cp_async8(&RG(S_QS, v), q + v * kp.ncells + offc);
+        if (ACCUM) cp_async8(&RG(S_ACC, v), rhs + v * kp.ncells + offs);
+        if (STAGE >= 1) cp_async8(&RG(S_QN, v), qnn + v * kp.ncells + offs);
+        if (STAGE >= 2) cp_async8(&RG(S_QS, v), q + v * kp.ncells + offs);
       }
       cp_async_commit();
     }
     double WL[NEQ], WR[NEQ];
 #pragma unroll
-    for (int v = 0; v < NEQ; ++v)
-      weno5(RG(sl, v), RG(s1, v), RG(s2, v), RG(s3, v), RG(s4, v), kp.eps4, WL[v], WR[v]);
-    double F[NEQ], uf = 0.0;
-    if (p >= 1) {
-      bad |= hllc<N, D, DIR>(kp, WLp, WR, F, uf);
-      if (p >= 2) {
-        const double du = (uf - ufp) * idx;
-        double r[NEQ];
+    for (int h = 0; h < NH; ++h) {
+      const double2 c = ld2(i1, h), dd = ld2(i2, h);
+      const double2 d1 = ld2(S_D * SLOT + i0, h), d2 = ld2(S_D * SLOT + i1, h), d3 = ld2(S_D * SLOT + i2, h);
+      const double2 u0 = ld2(S_U * SLOT + j0, h), u1 = ld2(S_U * SLOT + j1, h);
+      const bool two = 2 * h + 1 < NEQ;
+      double2 d4, u2;
+      d4.x = w[2 * h] - dd.x;
+      u2.x = weno5_u(d4.x - d3.x, kp.eps4);
+      d4.y = two ? w[two ? 2 * h + 1 : 0] - dd.y : 0.0;
+      u2.y = two ? weno5_u(d4.y - d3.y, kp.eps4) : 0.0;
+      st2(i0, h, make_double2(w[2 * h], two ? w[two ? 2 * h + 1 : 0] : 0.0));
+      st2(S_D * SLOT + i0, h, d4);
+      st2(S_U * SLOT + j0, h, u2);
+      weno5_core(c.x, d1.x, d2.x, d3.x, d4.x, u0.x, u1.x, u2.x, WL[2 * h], WR[2 * h]);
+      if (two) weno5_core(c.y, d1.y, d2.y, d3.y, d4.y, u0.y, u1.y, u2.y, WL[two ? 2 * h + 1 : 0], WR[two ? 2 * h + 1 : 0]);
+    }
+    {
+      const int t = i0;
+      i0 = i1, i1 = i2, i2 = t;
+      const int u = j0;
+      j0 = j1, j1 = u;
+    }
+    double F[NEQ], uf;
+    const bool fbad = hllc<N, D, DIR>(kp, WLp, WR, F, uf);  // face g-1/2: WL of cell g-1, WR of cell g
+    bad |= fbad && p >= 1;
+    if (p >= 2) {
+      const double du = (uf - ufp) * idx;
+      double r[NEQ];
 #pragma unroll
-        for (int v = 0; v < NEQ; ++v) {
-          r[v] = (Fp[v] - F[v]) * idx;
-          if (v >= IA) r[v] = fma(RG(s1, v), du, r[v]);
-        }
-        if (ACCUM || STAGE >= 1) cp_async_wait_all();
-        if (ACCUM) {
-#pragma unroll
-          for (int v = 0; v < NEQ; ++v) r[v] += RG(S_ACC, v);
-        }
-        if (STAGE >= 1) {
-          double qnc[NEQ], qsc[NEQ];
-#pragma unroll
-          for (int v = 0; v < NEQ; ++v) {
-            qnc[v] = RG(S_QN, v);
-            qsc[v] = STAGE >= 2 ? RG(S_QS, v) : 0.0;
-          }
-          rk_cell<N, D, STAGE>(kp, dt, qnc, qsc, r);
-        }
-        double* out = STAGE == 3 ? qnn : rhs;
-#pragma unroll
-        for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + offc] = r[v];
+      for (int v = 0; v < NEQ; ++v) {
+        r[v] = (Fp[v] - F[v]) * idx;
+        if (v >= IA) r[v] = fma(am[v - IA], du, r[v]);
       }
+      if (ACCUM || STAGE >= 1) cp_async_wait_all();
+      if (ACCUM) {
 #pragma unroll
-      for (int v = 0; v < NEQ; ++v) Fp[v] = F[v];
-      ufp = uf;
+        for (int h = 0; h < NH; ++h) {
+          const double2 a = ld2(S_ACC * SLOT, h);
+          r[2 * h] += a.x;
+          if (2 * h + 1 < NEQ) r[2 * h + 1 < NEQ ? 2 * h + 1 : 0] += a.y;
+        }
+      }
+      if (STAGE >= 1) {
+        double qnc[NEQ], qsc[NEQ];
+#pragma unroll
+        for (int h = 0; h < NH; ++h) {
+          const double2 a = ld2(S_QN * SLOT, h);
+          const double2 b = STAGE >= 2 ? ld2(S_QS * SLOT, h) : make_double2(0.0, 0.0);
+          qnc[2 * h] = a.x;
+          qsc[2 * h] = b.x;
+          if (2 * h + 1 < NEQ) {
+            qnc[2 * h + 1 < NEQ ? 2 * h + 1 : 0] = a.y;
+            qsc[2 * h + 1 < NEQ ? 2 * h + 1 : 0] = b.y;
+          }
+        }
+        rk_cell<N, D, STAGE>(kp, dt, qnc, qsc, r);
+      }
+      double* out = STAGE == 3 ? qnn : rhs;
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + offc] = r[v];
     }
 #pragma unroll
-    for (int v = 0; v < NEQ; ++v) WLp[v] = WL[v];
-    sl = s1;
+    for (int v = 0; v < NEQ; ++v) {
+      Fp[v] = F[v];
+      WLp[v] = WL[v];
+    }
+    ufp = uf;
+    offc += stride;
   }
 #undef RG
   if (bad) *kp.flag = 1;
@@ -581,7 +684,7 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, doubl
     const int nseg = (n + seglen - 1) / seglen;
     const long long threads = g->kp.ncells / n * nseg;
     const long long nb = (threads + MB - 1) / MB;
-    const size_t smem = sizeof(double) * march_slots(ACCUM, STAGE) * NEQ * MB;
+    const size_t smem = sizeof(double2) * march_slots(ACCUM, STAGE) * ((NEQ + 1) / 2) * MB;
     auto kern = sweep_march<N, D, DIR, ACCUM, STAGE>;
     static bool attr_done[16] = {};
     if (!attr_done[g->device & 15]) {
@@ -732,7 +835,7 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
     if ((p->bc_lo[d] == MFC_BC_PERIODIC) != (p->bc_hi[d] == MFC_BC_PERIODIC))
       return fail(MFC_ERR_ARG, "mfc_init_grid: periodic must be set on both ends of a direction");
     cells *= p->n[d];
-    if (cells > (1LL << 40)) return fail(MFC_ERR_ARG, "mfc_init_grid: grid too large");
+    if (cells >= (1LL << 31)) return fail(MFC_ERR_ARG, "mfc_init_grid: grid too large (cell offsets are 32-bit: fewer than 2^31 cells)");
   }
   for (int i = 0; i < p->nfluids; ++i)
     if (!(p->gamma[i] > 1.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: gamma_i must be > 1");

@@ -108,33 +108,60 @@ __device__ __forceinline__ bool prim_cell(const KP& kp, const double* q, double*
 //   * product form of the weights: a_r = d_r /(beta_r+eps)^2 is multiplied through by
 //     prod_j (beta_j+eps)^2, which leaves ONE reciprocal per reconstructed value and no other division;
 //   * beta_r and the three products are shared by the two values of the cell.
-__device__ __forceinline__ void weno5(double a, double b, double c, double d, double e, double eps4, double& L,
-                                      double& R) {
-  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
-  const double t0 = d2 - d1, t1 = d3 - d2, t2 = d4 - d3;
+// Split in two so that the y/z sweeps, which march along the stencil direction, can carry the per-cell
+// pieces (first differences d_k and u_k = 13/3 t_k^2 + 4 eps of the second differences t_k) from step to step
+// instead of recomputing them: weno5_u forms one u_k, weno5_core takes (c; d1..d4; u0..u2).
+// The coefficients live in constant memory so that they reach the FP64 instructions as constant-bank
+// operands: as literals ptxas re-materialises each of them with two UMOVs per loop iteration, and every
+// instruction that is not FP64 costs the sweeps an issue slot.
+enum { W_C133, W_03, W_06, W_01, W_5_60, W_M2_60, W_02, W_M005, W_M02, W_005, W_M01, W_2_60, W_M5_60, W_COUNT };
+#ifdef MFC_WC_LIT
+__device__ __forceinline__ constexpr double wc_lit(int i) {
+  constexpr double t[W_COUNT] = {13.0 / 3.0, 0.3, 0.6, 0.1, 5.0 / 60.0, -2.0 / 60.0, 0.2, -0.05, -0.2, 0.05, -0.1,
+                                 2.0 / 60.0, -5.0 / 60.0};
+  return t[i];
+}
+#define WCV(i) wc_lit(i)
+#else
+__constant__ double WC[W_COUNT] = {13.0 / 3.0, 0.3, 0.6, 0.1, 5.0 / 60.0, -2.0 / 60.0, 0.2, -0.05, -0.2, 0.05, -0.1,
+                                   2.0 / 60.0, -5.0 / 60.0};
+#define WCV(i) WC[i]
+#endif
+
+__device__ __forceinline__ double weno5_u(double t, double eps4) { return fma(WCV(W_C133) * t, t, eps4); }
+
+__device__ __forceinline__ void weno5_core(double c, double d1, double d2, double d3, double d4, double u0, double u1,
+                                           double u2, double& L, double& R) {
   const double s0 = fma(3.0, d2, -d1), s1 = d2 + d3, s2 = fma(-3.0, d3, d4);
-  constexpr double C133 = 13.0 / 3.0;
-  const double b0 = fma(C133 * t0, t0, fma(s0, s0, eps4));
-  const double b1 = fma(C133 * t1, t1, fma(s1, s1, eps4));
-  const double b2 = fma(C133 * t2, t2, fma(s2, s2, eps4));
+  const double b0 = fma(s0, s0, u0);
+  const double b1 = fma(s1, s1, u1);
+  const double b2 = fma(s2, s2, u2);
   const double e0 = b0 * b0, e1 = b1 * b1, e2 = b2 * b2;
   const double E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
   {  // ideal weights (1/10, 6/10, 3/10); candidates c + (5 d2 - 2 d1)/6, c + (d2 + 2 d3)/6, c + (4 d3 - d4)/6
-    const double S = fma(0.3, E01, fma(0.6, E02, 0.1 * E12));
-    const double Q0 = fma(5.0 / 60.0, d2, (-2.0 / 60.0) * d1);
-    const double Q1 = fma(0.1, d2, 0.2 * d3);
-    const double Q2 = fma(0.2, d3, -0.05 * d4);
+    const double S = fma(WCV(W_03), E01, fma(WCV(W_06), E02, WCV(W_01) * E12));
+    const double X = WCV(W_02) * d3;  // shared by Q1 and Q2
+    const double Q0 = fma(WCV(W_5_60), d2, WCV(W_M2_60) * d1);
+    const double Q1 = fma(WCV(W_01), d2, X);
+    const double Q2 = fma(WCV(W_M005), d4, X);
     const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
     L = fma(num, frcp(S), c);
   }
   {  // mirror image: ideal weights (3/10, 6/10, 1/10); c + (d1 - 4 d2)/6, c - (2 d2 + d3)/6, c + (2 d4 - 5 d3)/6
-    const double S = fma(0.1, E01, fma(0.6, E02, 0.3 * E12));
-    const double Q0 = fma(-0.2, d2, 0.05 * d1);
-    const double Q1 = fma(-0.2, d2, -0.1 * d3);
-    const double Q2 = fma(2.0 / 60.0, d4, (-5.0 / 60.0) * d3);
+    const double S = fma(WCV(W_01), E01, fma(WCV(W_06), E02, WCV(W_03) * E12));
+    const double Y = WCV(W_M02) * d2;  // shared by Q0 and Q1
+    const double Q0 = fma(WCV(W_005), d1, Y);
+    const double Q1 = fma(WCV(W_M01), d3, Y);
+    const double Q2 = fma(WCV(W_2_60), d4, WCV(W_M5_60) * d3);
     const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
     R = fma(num, frcp(S), c);
   }
+}
+
+__device__ __forceinline__ void weno5(double a, double b, double c, double d, double e, double eps4, double& L,
+                                      double& R) {
+  const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+  weno5_core(c, d1, d2, d3, d4, weno5_u(d2 - d1, eps4), weno5_u(d3 - d2, eps4), weno5_u(d4 - d3, eps4), L, R);
 }
 
 // O4 (S_L,S_R 653-654; S* 664; rho* 668; A5-A8): HLLC at one face with normal direction
