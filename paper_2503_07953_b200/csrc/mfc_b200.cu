@@ -29,7 +29,7 @@ constexpr unsigned FULL = 0xffffffffu;
 #define MFC_XW 4          // warps per block, sweep_x
 #endif
 #ifndef MFC_XMINB
-#define MFC_XMINB 1       // __launch_bounds__ min blocks per SM, sweep_x
+#define MFC_XMINB 3       // __launch_bounds__ min blocks per SM, sweep_x (168 registers: 12 warps per SM)
 #endif
 #ifndef MFC_MB
 #define MFC_MB 128        // threads per block, sweep_march
@@ -108,112 +108,127 @@ __device__ __forceinline__ void rk_cell(const KP& kp, double dt, const double* q
 // finished L of the cell goes straight through rk_cell and the new stage state is written instead of L —
 // stages 1 and 2 in place over the partial L in `rhs`, stage 3 over q^n in `qnn` (each cell of those buffers is
 // read and written by its one thread only; `q`, the state being swept, is never written).
+// Work items are (row, segment) pairs, item = row * nseg + segment; a warp owns a contiguous range of items and
+// walks through them as ONE stream of positions: the L+6 load positions of an item are followed directly by those of
+// the next, so that the two extra reconstruction positions per item cost 2/32 of a warp step instead of a whole
+// one (nx = 256: 8.2 steps per row instead of 9).  The grid is one wave of resident blocks (launch_x).
+struct XCursor {
+  int item, p, s0, nload, rowoff;  // position p of item `item`; s0, nload = L+6, rowoff = row*nx of that item
+};
+
 template <int N, int D, bool ACCUM, int STAGE>
 __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                    double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
   __shared__ double ring[XW][NEQ][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long wid = (long long)blockIdx.x * XW + warp;
+  const long long wid = (long long)blockIdx.x * XW + warp, nwarps = (long long)gridDim.x * XW;
   const int nx = kp.n[0];
-  const long long nrows = kp.ncells / nx;
-  if (wid >= nrows * nseg) return;  // warp-uniform
-  const int seg = (int)(wid % nseg);
-  const long long row = wid / nseg;
-  const int s0 = seg * seglen;
-  const int L = min(seglen, nx - s0);
-  const double* qrow = q + row * nx;
-  double* rrow = rhs + row * nx;
+  const long long nitems = kp.ncells / nx * nseg;
+  const int it0 = (int)(wid * nitems / nwarps), it1 = (int)((wid + 1) * nitems / nwarps);
+  if (it0 >= it1) return;  // warp-uniform
   double(*rg)[64] = ring[warp];
-  const int nload = L + 6, nrec = L + 2;
-  const int nsteps = (nrec + 31) >> 5, nchunks = (nload + 31) >> 5;
   const double idx = kp.inv_dx[0];
+  const int lo = kp.bc_lo[0], hi = kp.bc_hi[0];
   bool bad = false;
 
-  double qn[NEQ];
-  auto load = [&](int m) {
-    const int pos = 32 * m + lane;
-    if (pos < nload) {
-      const int g = ghost_index(s0 - 3 + pos, nx, kp.bc_lo[0], kp.bc_hi[0]);
-#pragma unroll
-      for (int v = 0; v < NEQ; ++v) qn[v] = __ldg(qrow + v * kp.ncells + g);
+  auto set_item = [&](XCursor& c) {
+    const int row = c.item / nseg;
+    c.s0 = (c.item - row * nseg) * seglen;
+    c.nload = min(seglen, nx - c.s0) + 6;
+    c.rowoff = row * nx;
+  };
+  auto advance = [&](XCursor& c, int by) {
+    c.p += by;
+    while (c.item < it1 && c.p >= c.nload) {
+      c.p -= c.nload;
+      ++c.item;
+      set_item(c);
     }
   };
-  auto store = [&](int m) {
-    const int pos = 32 * m + lane;
-    if (pos < nload) {
+  double qn[NEQ];
+  auto load = [&](const XCursor& c) {
+    if (c.item < it1) {
+      int g = c.s0 - 3 + c.p;  // O1: cells -3..nx+2
+      if (nx >= 3) {
+        if (g < 0) g = lo == BC_PERIODIC ? g + nx : 0;
+        if (g >= nx) g = hi == BC_PERIODIC ? g - nx : nx - 1;
+      } else {
+        g = ghost_index(g, nx, lo, hi);
+      }
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) qn[v] = __ldg(q + v * kp.ncells + (c.rowoff + g));
+    }
+  };
+  auto store = [&](const XCursor& c, int Q) {
+    if (c.item < it1) {
       double w[NEQ];
       bad |= prim_cell<N, D, false>(kp, qn, w);
 #pragma unroll
-      for (int v = 0; v < NEQ; ++v) rg[v][pos & 63] = w[v];
+      for (int v = 0; v < NEQ; ++v) rg[v][Q & 63] = w[v];
     }
   };
-  load(0);
-  store(0);
-  if (nchunks > 1) {
-    load(1);
-    store(1);
-  }
+  XCursor lc;  // load cursor: two chunks ahead of the reconstruction cursor
+  lc.item = it0;
+  lc.p = 0;
+  set_item(lc);
+  advance(lc, lane);
+  XCursor rc = lc;
+  load(lc);
+  store(lc, lane);
+  advance(lc, 32);
+  load(lc);
+  store(lc, 32 + lane);
+  advance(lc, 32);
   __syncwarp();
 
-  double WLc[NEQ], Fc[NEQ], ufc = 0.0;  // previous chunk's left states / fluxes (lane 31 feeds lane 0)
+  double WLc[NEQ], Fc[NEQ], ufc = 0.0;  // this lane's values of the previous step (lane 31 feeds lane 0)
 #pragma unroll
   for (int v = 0; v < NEQ; ++v) WLc[v] = Fc[v] = 0.0;
+  const int src = (lane + 31) & 31;
+  const bool last = lane == 31;
 
-  for (int c = 0; c < nsteps; ++c) {
-    const bool pre = c + 2 < nchunks;
-    if (pre) load(c + 2);
-    const int p = 32 * c + lane;
+  for (int Q = lane;; Q += 32) {
+    // a lane still has work if it is inside the reconstruction range of the last item or before that item
+    const bool more = rc.item < it1 - 1 || (rc.item == it1 - 1 && rc.p < rc.nload - 4);
+    if (!__any_sync(FULL, more)) break;
+    load(lc);
+    const int p = rc.p, nrec = rc.nload - 4;
+    const bool act = rc.item < it1 && p < nrec;
     double WL[NEQ], WR[NEQ];
 #pragma unroll
     for (int v = 0; v < NEQ; ++v)
-      weno5(rg[v][p & 63], rg[v][(p + 1) & 63], rg[v][(p + 2) & 63], rg[v][(p + 3) & 63], rg[v][(p + 4) & 63],
+      weno5(rg[v][Q & 63], rg[v][(Q + 1) & 63], rg[v][(Q + 2) & 63], rg[v][(Q + 3) & 63], rg[v][(Q + 4) & 63],
             kp.eps4, WL[v], WR[v]);
+    // left neighbour's value by a rotate: lane 31 sends what it had in the previous step
     double WLf[NEQ];
 #pragma unroll
     for (int v = 0; v < NEQ; ++v) {
-      const double up = __shfl_up_sync(FULL, WL[v], 1);
-      const double carry = __shfl_sync(FULL, WLc[v], 31);
-      WLf[v] = lane ? up : carry;
+      WLf[v] = __shfl_sync(FULL, last ? WLc[v] : WL[v], src);
       WLc[v] = WL[v];
     }
     double F[NEQ], uf;
     const bool fbad = hllc<N, D, 0>(kp, WLf, WR, F, uf);
-    if (p >= 1 && p < nrec) bad |= fbad;
+    if (act && p >= 1) bad |= fbad;
     double Fm[NEQ], ufm;
 #pragma unroll
     for (int v = 0; v < NEQ; ++v) {
-      const double up = __shfl_up_sync(FULL, F[v], 1);
-      const double carry = __shfl_sync(FULL, Fc[v], 31);
-      Fm[v] = lane ? up : carry;
+      Fm[v] = __shfl_sync(FULL, last ? Fc[v] : F[v], src);
       Fc[v] = F[v];
     }
-    {
-      const double up = __shfl_up_sync(FULL, uf, 1);
-      const double carry = __shfl_sync(FULL, ufc, 31);
-      ufm = lane ? up : carry;
-      ufc = uf;
-    }
-    if (p >= 2 && p < nrec) {  // cell i-1 = s0 + p - 2: eq.(10) and the alpha_i div(u) source
-      const int i = s0 + p - 2;
+    ufm = __shfl_sync(FULL, last ? ufc : uf, src);
+    ufc = uf;
+    if (act && p >= 2) {  // cell i = s0 + p - 2: eq.(10) and the alpha_i div(u) source
+      const int off = rc.rowoff + rc.s0 + p - 2;
       const double du = (uf - ufm) * idx;
-      if (STAGE == 0) {
+      double r[NEQ];
 #pragma unroll
-        for (int v = 0; v < NEQ; ++v) {
-          double r = (Fm[v] - F[v]) * idx;
-          if (v >= IA) r = fma(rg[v][(p + 1) & 63], du, r);
-          if (ACCUM) r += rrow[v * kp.ncells + i];
-          rrow[v * kp.ncells + i] = r;
-        }
-      } else {
-        double r[NEQ];
-#pragma unroll
-        for (int v = 0; v < NEQ; ++v) {
-          r[v] = (Fm[v] - F[v]) * idx;
-          if (v >= IA) r[v] = fma(rg[v][(p + 1) & 63], du, r[v]);
-          if (ACCUM) r[v] += rrow[v * kp.ncells + i];
-        }
-        const long long off = row * nx + i;
+      for (int v = 0; v < NEQ; ++v) {
+        r[v] = (Fm[v] - F[v]) * idx;
+        if (v >= IA) r[v] = fma(rg[v][(Q + 1) & 63], du, r[v]);
+        if (ACCUM) r[v] += rhs[v * kp.ncells + off];
+      }
+      if (STAGE >= 1) {
         double qnc[NEQ], qsc[NEQ];
 #pragma unroll
         for (int v = 0; v < NEQ; ++v) {
@@ -221,13 +236,15 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
           qsc[v] = STAGE >= 2 ? __ldg(q + v * kp.ncells + off) : 0.0;
         }
         rk_cell<N, D, STAGE>(kp, dt, qnc, qsc, r);
-        double* out = STAGE == 3 ? qnn : rhs;
-#pragma unroll
-        for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + off] = r[v];
       }
+      double* out = STAGE == 3 ? qnn : rhs;
+#pragma unroll
+      for (int v = 0; v < NEQ; ++v) out[v * kp.ncells + off] = r[v];
     }
     __syncwarp();
-    if (pre) store(c + 2);
+    store(lc, Q + 64);
+    advance(lc, 32);
+    advance(rc, 32);
     __syncwarp();
   }
   if (bad) *kp.flag = 1;
@@ -705,10 +722,21 @@ static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* q
   const int nx = g->kp.n[0];
   const int seglen = g->seg[0];
   const int nseg = (nx + seglen - 1) / seglen;
-  const long long warps = g->kp.ncells / nx * nseg;
-  const long long nb = (warps + XW - 1) / XW;
+  const long long items = g->kp.ncells / nx * nseg;
+  auto kern = sweep_x<N, D, ACCUM, STAGE>;
+  static int resident[16] = {};  // blocks per SM of this instantiation, per device
+  int& res = resident[g->device & 15];
+  if (res == 0) {
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&res, kern, XW * 32, 0);
+    if (e != cudaSuccess) return e;
+    if (res < 1) res = 1;
+  }
+  // one wave of resident blocks; every warp streams through a contiguous range of items
+  long long nb = (items + XW - 1) / XW;
+  const long long wave = (long long)res * g->num_sms;
+  if (nb > wave) nb = wave;
   Scope sc(g, MFC_K_SWEEP_X);
-  sweep_x<N, D, ACCUM, STAGE><<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt);
+  kern<<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt);
   return cudaGetLastError();
 }
 
