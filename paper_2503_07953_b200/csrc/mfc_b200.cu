@@ -14,6 +14,7 @@
 #include "../../include/mfc_b200.h"
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -118,19 +119,18 @@ struct XCursor {
 
 template <int N, int D, bool ACCUM, int STAGE>
 __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
-                                                   double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt) {
+                                                   double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt,
+                                                   int chunk, unsigned* next_chunk) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
   __shared__ double ring[XW][NEQ][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const long long wid = (long long)blockIdx.x * XW + warp, nwarps = (long long)gridDim.x * XW;
   const int nx = kp.n[0];
   const long long nitems = kp.ncells / nx * nseg;
-  const int it0 = (int)(wid * nitems / nwarps), it1 = (int)((wid + 1) * nitems / nwarps);
-  if (it0 >= it1) return;  // warp-uniform
   double(*rg)[64] = ring[warp];
   const double idx = kp.inv_dx[0];
   const int lo = kp.bc_lo[0], hi = kp.bc_hi[0];
   bool bad = false;
+  int it1 = 0;  // end of the current chunk of items
 
   auto set_item = [&](XCursor& c) {
     const int row = c.item / nseg;
@@ -168,6 +168,15 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
       for (int v = 0; v < NEQ; ++v) rg[v][Q & 63] = w[v];
     }
   };
+  // chunks of `chunk` consecutive items are handed out dynamically (one atomic per chunk), so that the warps of the
+  // single wave finish together
+  for (;;) {
+  unsigned ck = 0;
+  if (lane == 0) ck = atomicAdd(next_chunk, 1u);
+  ck = __shfl_sync(FULL, ck, 0);
+  if ((long long)ck * chunk >= nitems) break;
+  const int it0 = (int)ck * chunk;
+  it1 = (int)min((long long)it0 + chunk, nitems);
   XCursor lc;  // load cursor: two chunks ahead of the reconstruction cursor
   lc.item = it0;
   lc.p = 0;
@@ -246,6 +255,7 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
     advance(lc, 32);
     advance(rc, 32);
     __syncwarp();
+  }
   }
   if (bad) *kp.flag = 1;
 }
@@ -578,6 +588,8 @@ struct mfc_grid {
   double* hr = nullptr;
   unsigned long long* d_red = nullptr;  // [0] = smax bits
   int* d_flag = nullptr;
+  unsigned* d_xnext = nullptr;          // work counter of sweep_x
+  int xchunk = 0;                       // items per chunk (0 = default)
   unsigned long long* h_red = nullptr;  // pinned: [0] smax bits, [1] flag
   int seg[3];
   long long launches = 0;
@@ -731,12 +743,19 @@ static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* q
     if (e != cudaSuccess) return e;
     if (res < 1) res = 1;
   }
-  // one wave of resident blocks; every warp streams through a contiguous range of items
+  // one wave of resident blocks; the warps take chunks of consecutive items from a counter until none is left
   long long nb = (items + XW - 1) / XW;
   const long long wave = (long long)res * g->num_sms;
   if (nb > wave) nb = wave;
+  // chunk: about 8 chunks per warp for balance, at least 1 item, at most 16 (longer streams gain nothing)
+  long long chunk = items / (nb * XW * 8);
+  if (chunk < 1) chunk = 1;
+  if (chunk > 16) chunk = 16;
+  if (g->xchunk > 0) chunk = g->xchunk;
+  cudaError_t e = cudaMemsetAsync(g->d_xnext, 0, sizeof(unsigned), g->stream);
+  if (e != cudaSuccess) return e;
   Scope sc(g, MFC_K_SWEEP_X);
-  kern<<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt);
+  kern<<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt, (int)chunk, g->d_xnext);
   return cudaGetLastError();
 }
 
@@ -900,11 +919,13 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, p->device) == cudaSuccess) g->num_sms = prop.multiProcessorCount;
   default_segments(g);
+  if (const char* xc = std::getenv("MFC_XCHUNK")) g->xchunk = std::atoi(xc);  // tuning knob (benchmarks only)
 
   const size_t bytes = state_bytes(g);
   cudaError_t e;
   if ((e = cudaMalloc(&g->q1, bytes)) != cudaSuccess || (e = cudaMalloc(&g->Lq, bytes)) != cudaSuccess ||
       (e = cudaMalloc(&g->d_red, 16)) != cudaSuccess || (e = cudaMalloc(&g->d_flag, sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc(&g->d_xnext, sizeof(unsigned))) != cudaSuccess ||
       (e = cudaMallocHost(&g->h_red, 16)) != cudaSuccess) {
     mfc_free_grid(g);
     g_err = std::string("mfc_init_grid: allocation failed: ") + cudaGetErrorString(e);
@@ -928,6 +949,7 @@ mfc_status mfc_free_grid(mfc_grid* g) {
   cudaFree(g->hr);
   cudaFree(g->d_red);
   cudaFree(g->d_flag);
+  cudaFree(g->d_xnext);
   if (g->h_red) cudaFreeHost(g->h_red);
   drain_profile(g);
   for (cudaEvent_t e : g->pool) cudaEventDestroy(e);
