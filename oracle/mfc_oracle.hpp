@@ -37,7 +37,9 @@ constexpr int kMaxFluids = 4;
 constexpr int kMaxEq = 2 * kMaxFluids + 3 + 1;
 
 enum { BC_PERIODIC = 0, BC_EXTRAP = 1 };
-enum { RECON_PIECEWISE_CONSTANT = 1, RECON_WENO5_JS = 5 };
+// RECON_WENO5_M: mapped weights of Henrick et al. (the paper's ref. [30]);
+// RECON_WENO5_Z: WENO-Z weights (§4.2.2) with q = 1.
+enum { RECON_PIECEWISE_CONSTANT = 1, RECON_WENO5_JS = 5, RECON_WENO5_M = 6, RECON_WENO5_Z = 7 };
 
 // generic helpers so that T may be double, long double or the counting type
 template <class T> inline T o_sqrt(const T& x) { using std::sqrt; return sqrt(x); }
@@ -163,6 +165,62 @@ void weno5_js(const T& a, const T& b, const T& c, const T& d, const T& e, const 
     T a2 = o_ratio<T>(1, 10) / ((b2 + eps) * (b2 + eps));
     T s = a0 + a1 + a2;
     *right = c + ((a0 / s) * P0 + (a1 / s) * P1 + (a2 / s) * P2);
+  }
+}
+
+// O3-M / O3-Z: the same candidates, smoothness indicators and ideal weights as weno5_js; only the step from
+// (d_r, beta_r) to the nonlinear weights omega_r differs.
+//   RECON_WENO5_JS  alpha_r = d_r/(beta_r+eps)^2,                 omega_r = alpha_r / sum alpha
+//   RECON_WENO5_M   omega*_r = the JS weights; g_r(w) = w (d_r + d_r^2 - 3 d_r w + w^2) / (d_r^2 + w (1 - 2 d_r));
+//                   omega_r = g_r(omega*_r) / sum_s g_s(omega*_s)    ("mapped weights, following Henrick et al.",
+//                   PAPER.md:165; the map itself is not printed in the paper, reading A20)
+//   RECON_WENO5_Z   tau = |beta_0 - beta_2|, alpha_r = d_r (1 + (tau/(beta_r+eps))^q), q = 1,
+//                   omega_r = alpha_r / sum alpha
+template <class T>
+void weno5_weights(int recon, const T dr[3], const T beta[3], const T& eps, T omega[3]) {
+  T al[3];
+  if (recon == RECON_WENO5_Z) {
+    const T tau = o_abs(beta[0] - beta[2]);
+    for (int r = 0; r < 3; ++r) al[r] = dr[r] * (T(1) + tau / (beta[r] + eps));
+  } else {
+    for (int r = 0; r < 3; ++r) al[r] = dr[r] / ((beta[r] + eps) * (beta[r] + eps));
+  }
+  T s = al[0] + al[1] + al[2];
+  for (int r = 0; r < 3; ++r) omega[r] = al[r] / s;
+  if (recon == RECON_WENO5_M) {
+    T g[3];
+    for (int r = 0; r < 3; ++r) {
+      const T w = omega[r], d = dr[r];
+      g[r] = (w * (d + d * d - T(3) * d * w + w * w)) / (d * d + w * (T(1) - T(2) * d));
+    }
+    T sg = g[0] + g[1] + g[2];
+    for (int r = 0; r < 3; ++r) omega[r] = g[r] / sg;
+  }
+}
+
+// Stencil, outputs and evaluation form exactly as weno5_js (which it reproduces for recon = RECON_WENO5_JS up to
+// the order of two roundings: here omega_r is formed before it multiplies the candidate).
+template <class T>
+void weno5(int recon, const T& a, const T& b, const T& c, const T& d, const T& e, const T& eps, T* left, T* right) {
+  const T c1312 = o_ratio<T>(13, 12), c14 = o_ratio<T>(1, 4);
+  T t0 = a - T(2) * b + c, t1 = b - T(2) * c + d, t2 = c - T(2) * d + e;
+  T s0 = a - T(4) * b + T(3) * c, s1 = b - d, s2 = T(3) * c - T(4) * d + e;
+  T beta[3] = {c1312 * (t0 * t0) + c14 * (s0 * s0), c1312 * (t1 * t1) + c14 * (s1 * s1),
+               c1312 * (t2 * t2) + c14 * (s2 * s2)};
+  T d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
+  {  // left-biased value at i+1/2, ideal weights (1/10, 6/10, 3/10)
+    const T dr[3] = {o_ratio<T>(1, 10), o_ratio<T>(6, 10), o_ratio<T>(3, 10)};
+    T P0 = (T(5) * d2 - T(2) * d1) / T(6), P1 = (d2 + T(2) * d3) / T(6), P2 = (T(4) * d3 - d4) / T(6);
+    T om[3];
+    weno5_weights(recon, dr, beta, eps, om);
+    *left = c + (om[0] * P0 + om[1] * P1 + om[2] * P2);
+  }
+  {  // right-biased value at i-1/2 (mirror image), ideal weights (3/10, 6/10, 1/10), same beta
+    const T dr[3] = {o_ratio<T>(3, 10), o_ratio<T>(6, 10), o_ratio<T>(1, 10)};
+    T P0 = (d1 - T(4) * d2) / T(6), P1 = (T(0) - (T(2) * d2 + d3)) / T(6), P2 = (T(2) * d4 - T(5) * d3) / T(6);
+    T om[3];
+    weno5_weights(recon, dr, beta, eps, om);
+    *right = c + (om[0] * P0 + om[1] * P1 + om[2] * P2);
   }
 }
 
@@ -309,6 +367,8 @@ struct Solver {
             T l, r;
             if (P.recon == RECON_WENO5_JS) {
               weno5_js(c[-2 * neq], c[-neq], c[0], c[neq], c[2 * neq], P.weno_eps, &l, &r);
+            } else if (P.recon == RECON_WENO5_M || P.recon == RECON_WENO5_Z) {
+              weno5(P.recon, c[-2 * neq], c[-neq], c[0], c[neq], c[2 * neq], P.weno_eps, &l, &r);
             } else {  // PAPER.md:155-157 piecewise constant
               l = c[0]; r = c[0];
             }

@@ -123,6 +123,23 @@ void oracle_weno5_js_ld(const double* s, double eps, double* left, double* right
   *right = double(r);
 }
 
+// weights variant `recon` (RECON_WENO5_JS / _M / _Z) of the general routine, fp64 and 80-bit
+void oracle_weno5(int recon, const double* s, double eps, double* left, double* right) {
+  weno5<double>(recon, s[0], s[1], s[2], s[3], s[4], eps, left, right);
+}
+
+void oracle_weno5_ld(int recon, const double* s, double eps, double* left, double* right) {
+  long double l, r;
+  weno5<long double>(recon, s[0], s[1], s[2], s[3], s[4], (long double)eps, &l, &r);
+  *left = double(l);
+  *right = double(r);
+}
+
+// the weights step alone: omega[3] from ideal weights dr[3] and smoothness indicators beta[3]
+void oracle_weno5_weights(int recon, const double* dr, const double* beta, double eps, double* omega) {
+  weno5_weights<double>(recon, dr, beta, eps, omega);
+}
+
 int oracle_hllc_face(const oracle_params* p, int dir, const double* wL, const double* wR, double* F, double* uf) {
   return hllc_face<double>(convert<double>(p), dir, wL, wR, F, uf);
 }

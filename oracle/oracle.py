@@ -13,6 +13,8 @@ from . import build as _build
 
 BC_PERIODIC, BC_EXTRAP = 0, 1
 RECON_PC, RECON_WENO5 = 1, 5
+RECON_WENO5_M, RECON_WENO5_Z = 6, 7   # mapped (Henrick) and WENO-Z weights
+RECON_BY_NAME = {"js": RECON_WENO5, "m": RECON_WENO5_M, "z": RECON_WENO5_Z}
 _MAXF = 4
 
 
@@ -42,6 +44,9 @@ def lib():
         L.oracle_cfl_dt.argtypes = [pp, dp, C.c_double]; L.oracle_cfl_dt.restype = C.c_double
         L.oracle_weno5_js.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js.restype = None
         L.oracle_weno5_js_ld.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js_ld.restype = None
+        L.oracle_weno5.argtypes = [C.c_int, dp, C.c_double, dp, dp]; L.oracle_weno5.restype = None
+        L.oracle_weno5_ld.argtypes = [C.c_int, dp, C.c_double, dp, dp]; L.oracle_weno5_ld.restype = None
+        L.oracle_weno5_weights.argtypes = [C.c_int, dp, dp, C.c_double, dp]; L.oracle_weno5_weights.restype = None
         L.oracle_hllc_face.argtypes = [pp, C.c_int, dp, dp, dp, dp]
         L.oracle_clamp_cell.argtypes = [pp, dp]; L.oracle_clamp_cell.restype = None
         L.oracle_rhs_ld.argtypes = [pp, dp, dp, C.c_int]; L.oracle_rhs_ld.restype = C.c_long
@@ -56,8 +61,10 @@ def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def make_params(case, recon=RECON_WENO5):
-    """case: a workloads.Case (n, dx, gamma, pi_inf, bc_lo, bc_hi, weno_eps, alpha_floor, clamp)."""
+def make_params(case, recon=None):
+    """case: a workloads.Case (n, dx, gamma, pi_inf, bc_lo, bc_hi, weno_eps, alpha_floor, clamp[, weno])."""
+    if recon is None:
+        recon = RECON_BY_NAME[getattr(case, "weno", "js")]
     p = OracleParams()
     p.ndim = case.ndim
     for d in range(3):
@@ -79,7 +86,7 @@ def make_params(case, recon=RECON_WENO5):
 class Oracle:
     """The five operations of include/mfc_b200.h on host numpy arrays (SoA, x fastest)."""
 
-    def __init__(self, case, recon=RECON_WENO5):
+    def __init__(self, case, recon=None):
         self.case = case
         self.p = make_params(case, recon)
         self.neq = 2 * case.nfluids + case.ndim + 1
@@ -136,6 +143,22 @@ def weno5_js(s, eps):
     l, r = C.c_double(), C.c_double()
     lib().oracle_weno5_js(_dp(s), float(eps), C.byref(l), C.byref(r))
     return l.value, r.value
+
+
+def weno5(recon, s, eps, ld=False):
+    """general routine with the weights variant `recon`; ld: the same text in 80-bit arithmetic"""
+    s = np.ascontiguousarray(s, dtype=np.float64)
+    l, r = C.c_double(), C.c_double()
+    (lib().oracle_weno5_ld if ld else lib().oracle_weno5)(int(recon), _dp(s), float(eps), C.byref(l), C.byref(r))
+    return l.value, r.value
+
+
+def weno5_weights(recon, dr, beta, eps):
+    dr = np.ascontiguousarray(dr, dtype=np.float64)
+    beta = np.ascontiguousarray(beta, dtype=np.float64)
+    om = np.empty(3)
+    lib().oracle_weno5_weights(int(recon), _dp(dr), _dp(beta), float(eps), _dp(om))
+    return om
 
 
 def weno5_js_ld(s, eps):
