@@ -57,6 +57,12 @@ typedef enum {
  * (the paper's Taylor-Green case, implies it).  Periodic must be set on both ends. */
 typedef enum { MFC_BC_PERIODIC = 0, MFC_BC_EXTRAP = 1 } mfc_bc;
 
+/* Nonlinear weights of the fifth-order WENO reconstruction.  JS: alpha_r = d_r/(beta_r+eps)^2
+ * (the weights BASELINE.json names).  M: the JS weights passed through the map of Henrick et al. and
+ * renormalised ("mapped weights", PAPER.md:165 — the paper's default).  Z: alpha_r = d_r (1 + tau/(beta_r+eps)),
+ * tau = |beta_0 - beta_2| (PAPER.md:562-566 with q = 1). */
+typedef enum { MFC_WENO_JS = 0, MFC_WENO_M = 1, MFC_WENO_Z = 2 } mfc_weno;
+
 #define MFC_MAX_FLUIDS 3
 
 typedef struct {
@@ -70,6 +76,7 @@ typedef struct {
   double weno_eps;       /* epsilon of the WENO weights, PAPER.md:163/566 (A4); > 0 */
   double alpha_floor;    /* volume-fraction floor of the RK-stage clamp (A10) */
   int clamp;             /* 0: no clamp; 1: apply A10 after every RK stage */
+  int weno;              /* mfc_weno: nonlinear weights of the reconstruction; 0 = MFC_WENO_JS */
   int device;            /* CUDA device ordinal */
   void *stream;          /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
 } mfc_params;

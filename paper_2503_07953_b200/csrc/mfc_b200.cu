@@ -117,7 +117,7 @@ struct XCursor {
   int item, p, s0, nload, rowoff;  // position p of item `item`; s0, nload = L+6, rowoff = row*nx of that item
 };
 
-template <int N, int D, bool ACCUM, int STAGE>
+template <int N, int D, bool ACCUM, int STAGE, int WV>
 __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                    double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt,
                                                    int chunk, unsigned* next_chunk) {
@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
     double WL[NEQ], WR[NEQ];
 #pragma unroll
     for (int v = 0; v < NEQ; ++v)
-      weno5(rg[v][Q & 63], rg[v][(Q + 1) & 63], rg[v][(Q + 2) & 63], rg[v][(Q + 3) & 63], rg[v][(Q + 4) & 63],
+      weno5<WV>(rg[v][Q & 63], rg[v][(Q + 1) & 63], rg[v][(Q + 2) & 63], rg[v][(Q + 3) & 63], rg[v][(Q + 4) & 63],
             kp.eps4, WL[v], WR[v]);
     // left neighbour's value by a rotate: lane 31 sends what it had in the previous step
     double WLf[NEQ];
@@ -280,7 +280,7 @@ __host__ __device__ constexpr int march_slots(bool accum, int stage) {
   return MARCH_RING + (accum ? 1 : 0) + (stage >= 1 ? 1 : 0) + (stage >= 2 ? 1 : 0);
 }
 
-template <int N, int D, int DIR, bool ACCUM, int STAGE>
+template <int N, int D, int DIR, bool ACCUM, int STAGE, int WV>
 __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                   double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
@@ -432,8 +432,8 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
       st2(i0, h, make_double2(w[2 * h], two ? w[two ? 2 * h + 1 : 0] : 0.0));
       st2(S_D * SLOT + i0, h, d4);
       st2(S_U * SLOT + j0, h, u2);
-      weno5_core(c.x, d1.x, d2.x, d3.x, d4.x, u0.x, u1.x, u2.x, WL[2 * h], WR[2 * h]);
-      if (two) weno5_core(c.y, d1.y, d2.y, d3.y, d4.y, u0.y, u1.y, u2.y, WL[two ? 2 * h + 1 : 0], WR[two ? 2 * h + 1 : 0]);
+      weno5_core<WV>(c.x, d1.x, d2.x, d3.x, d4.x, u0.x, u1.x, u2.x, WL[2 * h], WR[2 * h]);
+      if (two) weno5_core<WV>(c.y, d1.y, d2.y, d3.y, d4.y, u0.y, u1.y, u2.y, WL[two ? 2 * h + 1 : 0], WR[two ? 2 * h + 1 : 0]);
     }
     {
       const int t = i0;
@@ -543,12 +543,13 @@ __global__ void __launch_bounds__(PB) cfl_kernel(const __grid_constant__ KP kp, 
 }
 
 // ------------------------------------------------------------------------------------------------ unit entry points
+template <int WV>
 __global__ void __launch_bounds__(PB) weno5_unit_kernel(const __grid_constant__ KP kp, const double* __restrict__ s,
                                                         long long count, double* left, double* right) {
   const long long t = (long long)blockIdx.x * PB + threadIdx.x;
   if (t >= count) return;
   double L, R;
-  weno5(s[5 * t], s[5 * t + 1], s[5 * t + 2], s[5 * t + 3], s[5 * t + 4], kp.eps4, L, R);
+  weno5<WV>(s[5 * t], s[5 * t + 1], s[5 * t + 2], s[5 * t + 3], s[5 * t + 4], kp.eps4, L, R);
   left[t] = L;
   right[t] = R;
 }
@@ -580,6 +581,7 @@ using namespace mfc;
 struct mfc_grid {
   KP kp;
   int ndim, nf, neq;
+  int weno = 0;  // WENO_JS / WENO_M / WENO_Z
   int device;
   cudaStream_t stream;
   double* q1 = nullptr;     // stage state
@@ -704,7 +706,7 @@ static cudaError_t launch_prim(mfc_grid* g, const double* q, double* w) {
   return cudaGetLastError();
 }
 
-template <int N, int D, int DIR, bool ACCUM, int STAGE>
+template <int N, int D, int WV, int DIR, bool ACCUM, int STAGE>
 static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, double* qn, double dt) {
   if constexpr (DIR < D) {
     constexpr int NEQ = 2 * N + D + 1;
@@ -714,7 +716,7 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, doubl
     const long long threads = g->kp.ncells / n * nseg;
     const long long nb = (threads + MB - 1) / MB;
     const size_t smem = sizeof(double2) * march_slots(ACCUM, STAGE) * ((NEQ + 1) / 2) * MB;
-    auto kern = sweep_march<N, D, DIR, ACCUM, STAGE>;
+    auto kern = sweep_march<N, D, DIR, ACCUM, STAGE, WV>;
     static bool attr_done[16] = {};
     if (!attr_done[g->device & 15]) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -729,13 +731,13 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, doubl
   }
 }
 
-template <int N, int D, bool ACCUM, int STAGE>
+template <int N, int D, int WV, bool ACCUM, int STAGE>
 static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* qn, double dt) {
   const int nx = g->kp.n[0];
   const int seglen = g->seg[0];
   const int nseg = (nx + seglen - 1) / seglen;
   const long long items = g->kp.ncells / nx * nseg;
-  auto kern = sweep_x<N, D, ACCUM, STAGE>;
+  auto kern = sweep_x<N, D, ACCUM, STAGE, WV>;
   static int resident[16] = {};  // blocks per SM of this instantiation, per device
   int& res = resident[g->device & 15];
   if (res == 0) {
@@ -760,39 +762,39 @@ static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* q
 }
 
 // rhs = L(q) restricted to the directions in mask.  mask == all: x overwrites, y and z accumulate.
-template <int N, int D>
+template <int N, int D, int WV>
 static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mask) {
   const int all = (1 << D) - 1;
   cudaError_t e;
   if ((mask & all) == all) {
-    if ((e = launch_x<N, D, false, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
+    if ((e = launch_x<N, D, WV, false, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   } else {
     if ((e = cudaMemsetAsync(rhs, 0, state_bytes(g), g->stream)) != cudaSuccess) return e;
     if (mask & 1)
-      if ((e = launch_x<N, D, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
+      if ((e = launch_x<N, D, WV, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   }
   if (D >= 2 && (mask & 2))
-    if ((e = launch_march<N, D, 1, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
+    if ((e = launch_march<N, D, WV, 1, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   if (D >= 3 && (mask & 4))
-    if ((e = launch_march<N, D, 2, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
+    if ((e = launch_march<N, D, WV, 2, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   return cudaSuccess;
 }
 
 // One RK stage: L(qs) by the D sweeps, the last of which applies the stage combination and the clamp itself
 // (no separate RK kernel, the finished L never goes to HBM).  Stages 1 and 2 leave the new stage state in `work`
 // (where the partial L was), stage 3 writes q^{n+1} over q^n.
-template <int N, int D, int STAGE>
+template <int N, int D, int WV, int STAGE>
 static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, double* qn, double dt) {
   cudaError_t e;
   if constexpr (D == 1) {
-    return launch_x<N, D, false, STAGE>(g, qs, work, qn, dt);
+    return launch_x<N, D, WV, false, STAGE>(g, qs, work, qn, dt);
   } else {
-    if ((e = launch_x<N, D, false, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
+    if ((e = launch_x<N, D, WV, false, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
     if constexpr (D == 2) {
-      return launch_march<N, D, 1, true, STAGE>(g, qs, work, qn, dt);
+      return launch_march<N, D, WV, 1, true, STAGE>(g, qs, work, qn, dt);
     } else {
-      if ((e = launch_march<N, D, 1, true, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
-      return launch_march<N, D, 2, true, STAGE>(g, qs, work, qn, dt);
+      if ((e = launch_march<N, D, WV, 1, true, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
+      return launch_march<N, D, WV, 2, true, STAGE>(g, qs, work, qn, dt);
     }
   }
 }
@@ -800,12 +802,12 @@ static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, dou
 // O6: q^n in `q` (caller's), two work arrays A = Lq, B = q1:
 //   stage 1 sweeps q,  partial L in A, q1 ends in A;   stage 2 sweeps A, partial L in B, q2 ends in B;
 //   stage 3 sweeps B,  partial L in A, q^{n+1} ends in q.
-template <int N, int D>
+template <int N, int D, int WV>
 static cudaError_t launch_rk3(mfc_grid* g, double* q, double dt) {
   cudaError_t e;
-  if ((e = launch_stage<N, D, 1>(g, q, g->Lq, q, dt)) != cudaSuccess) return e;
-  if ((e = launch_stage<N, D, 2>(g, g->Lq, g->q1, q, dt)) != cudaSuccess) return e;
-  return launch_stage<N, D, 3>(g, g->q1, g->Lq, q, dt);
+  if ((e = launch_stage<N, D, WV, 1>(g, q, g->Lq, q, dt)) != cudaSuccess) return e;
+  if ((e = launch_stage<N, D, WV, 2>(g, g->Lq, g->q1, q, dt)) != cudaSuccess) return e;
+  return launch_stage<N, D, WV, 3>(g, g->q1, g->Lq, q, dt);
 }
 
 template <int N, int D>
@@ -857,6 +859,25 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
   }()
 #endif
 
+// the same with the weights variant WV of the handle as a third compile-time constant
+#ifdef MFC_ONLY_23
+#define MFC_DISPATCH_W(g, EXPR)                                                   \
+  [&]() -> cudaError_t {                                                          \
+    constexpr int WV = WENO_JS;                                                   \
+    return (g)->weno == WENO_JS ? MFC_DISPATCH(g, EXPR) : cudaErrorInvalidValue;  \
+  }()
+#else
+#define MFC_DISPATCH_W(g, EXPR)                                                   \
+  [&]() -> cudaError_t {                                                          \
+    switch ((g)->weno) {                                                          \
+      case WENO_JS: { constexpr int WV = WENO_JS; return MFC_DISPATCH(g, EXPR); } \
+      case WENO_M: { constexpr int WV = WENO_M; return MFC_DISPATCH(g, EXPR); }   \
+      case WENO_Z: { constexpr int WV = WENO_Z; return MFC_DISPATCH(g, EXPR); }   \
+    }                                                                             \
+    return cudaErrorInvalidValue;                                                 \
+  }()
+#endif
+
 static mfc_status use_device(const mfc_grid* g) {
   CK(cudaSetDevice(g->device));
   return MFC_OK;
@@ -887,6 +908,8 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   for (int i = 0; i < p->nfluids; ++i)
     if (!(p->gamma[i] > 1.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: gamma_i must be > 1");
   if (!(p->weno_eps > 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: weno_eps must be > 0");
+  if (p->weno != MFC_WENO_JS && p->weno != MFC_WENO_M && p->weno != MFC_WENO_Z)
+    return fail(MFC_ERR_ARG, "mfc_init_grid: weno must be MFC_WENO_JS, MFC_WENO_M or MFC_WENO_Z");
   int ndev = 0;
   CK(cudaGetDeviceCount(&ndev));
   if (p->device < 0 || p->device >= ndev) return fail(MFC_ERR_ARG, "mfc_init_grid: no such CUDA device");
@@ -897,6 +920,7 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   std::memset(&g->kp, 0, sizeof(KP));
   g->ndim = p->ndim;
   g->nf = p->nfluids;
+  g->weno = p->weno;
   g->neq = 2 * p->nfluids + p->ndim + 1;
   g->device = p->device;
   g->stream = (cudaStream_t)p->stream;
@@ -982,7 +1006,7 @@ mfc_status mfc_rhs_dirs(mfc_grid* g, const double* q, double* rhs, int dir_mask)
   if (!g || !q || !rhs) return fail(MFC_ERR_ARG, "mfc_rhs: NULL argument");
   if (q == rhs) return fail(MFC_ERR_ARG, "mfc_rhs: q and rhs must not alias");
   if (mfc_status s = use_device(g)) return s;
-  CK(MFC_DISPATCH(g, (launch_rhs<N, D>(g, q, rhs, dir_mask))));
+  CK(MFC_DISPATCH_W(g, (launch_rhs<N, D, WV>(g, q, rhs, dir_mask))));
   return MFC_OK;
 }
 
@@ -993,7 +1017,7 @@ mfc_status mfc_rk3_steps(mfc_grid* g, double* q, double dt, int nsteps) {
   if (nsteps < 0) return fail(MFC_ERR_ARG, "mfc_rk3_steps: nsteps < 0");
   if (!(dt == dt)) return fail(MFC_ERR_ARG, "mfc_rk3_step: dt is NaN");
   if (mfc_status s = use_device(g)) return s;
-  for (int s = 0; s < nsteps; ++s) CK(MFC_DISPATCH(g, (launch_rk3<N, D>(g, q, dt))));
+  for (int s = 0; s < nsteps; ++s) CK(MFC_DISPATCH_W(g, (launch_rk3<N, D, WV>(g, q, dt))));
   return MFC_OK;
 }
 
@@ -1049,7 +1073,7 @@ mfc_status mfc_rhs_host(mfc_grid* g, const double* q_host, double* rhs_host) {
   if (mfc_status s = use_device(g)) return s;
   if (mfc_status s = ensure_staging(g, true)) return s;
   CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));
-  CK(MFC_DISPATCH(g, (launch_rhs<N, D>(g, g->hq, g->hr, 7))));
+  CK(MFC_DISPATCH_W(g, (launch_rhs<N, D, WV>(g, g->hq, g->hr, 7))));
   CK(cudaMemcpyAsync(rhs_host, g->hr, state_bytes(g), cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   return MFC_OK;
@@ -1061,7 +1085,7 @@ mfc_status mfc_rk3_steps_host(mfc_grid* g, double* q_host, double dt, int nsteps
   if (mfc_status s = use_device(g)) return s;
   if (mfc_status s = ensure_staging(g, false)) return s;
   CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));
-  for (int s = 0; s < nsteps; ++s) CK(MFC_DISPATCH(g, (launch_rk3<N, D>(g, g->hq, dt))));
+  for (int s = 0; s < nsteps; ++s) CK(MFC_DISPATCH_W(g, (launch_rk3<N, D, WV>(g, g->hq, dt))));
   CK(cudaMemcpyAsync(q_host, g->hq, state_bytes(g), cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   return MFC_OK;
@@ -1072,7 +1096,7 @@ static mfc_status advance_impl(mfc_grid* g, double* q, double cfl, int nsteps, d
   for (int s = 0; s < nsteps; ++s) {
     double dt = 0.0;
     if (mfc_status st = mfc_cfl_dt(g, q, cfl, &dt)) return st;
-    CK(MFC_DISPATCH(g, (launch_rk3<N, D>(g, q, dt))));
+    CK(MFC_DISPATCH_W(g, (launch_rk3<N, D, WV>(g, q, dt))));
     t += dt;
   }
   if (t_out) *t_out = t;
@@ -1105,7 +1129,10 @@ mfc_status mfc_weno5_values(mfc_grid* g, const double* stencils, long long count
   if (count == 0) return MFC_OK;
   {
     Scope sc(g, MFC_K_PRIM);
-    weno5_unit_kernel<<<(unsigned)((count + PB - 1) / PB), PB, 0, g->stream>>>(g->kp, stencils, count, left, right);
+    const unsigned nb = (unsigned)((count + PB - 1) / PB);
+    if (g->weno == WENO_M) weno5_unit_kernel<WENO_M><<<nb, PB, 0, g->stream>>>(g->kp, stencils, count, left, right);
+    else if (g->weno == WENO_Z) weno5_unit_kernel<WENO_Z><<<nb, PB, 0, g->stream>>>(g->kp, stencils, count, left, right);
+    else weno5_unit_kernel<WENO_JS><<<nb, PB, 0, g->stream>>>(g->kp, stencils, count, left, right);
   }
   CK(cudaGetLastError());
   return MFC_OK;

@@ -7,6 +7,7 @@
 namespace mfc {
 
 enum { BC_PERIODIC = 0, BC_EXTRAP = 1 };
+enum { WENO_JS = 0, WENO_M = 1, WENO_Z = 2 };  // nonlinear weights (mfc_weno of include/mfc_b200.h)
 
 // Kernel parameters (passed by value; lives in the constant bank of each launch).
 struct KP {
@@ -130,38 +131,82 @@ __constant__ double WC[W_COUNT] = {13.0 / 3.0, 0.3, 0.6, 0.1, 5.0 / 60.0, -2.0 /
 
 __device__ __forceinline__ double weno5_u(double t, double eps4) { return fma(WCV(W_C133) * t, t, eps4); }
 
+// One reconstructed value c + sum_r A_r Q_r / sum_r A_r from unnormalised weights A_r that already hold the ideal
+// weights' ratios (A = (A0, A1, A2) for stencils 0, 1, 2) and the candidate deviations Q_r scaled by the same
+// constants — see weno5_core for the JS/Z case.  One reciprocal.
+template <int WV>
 __device__ __forceinline__ void weno5_core(double c, double d1, double d2, double d3, double d4, double u0, double u1,
                                            double u2, double& L, double& R) {
   const double s0 = fma(3.0, d2, -d1), s1 = d2 + d3, s2 = fma(-3.0, d3, d4);
-  const double b0 = fma(s0, s0, u0);
+  const double b0 = fma(s0, s0, u0);  // 4 (beta_r + eps)
   const double b1 = fma(s1, s1, u1);
   const double b2 = fma(s2, s2, u2);
-  const double e0 = b0 * b0, e1 = b1 * b1, e2 = b2 * b2;
-  const double E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
-  {  // ideal weights (1/10, 6/10, 3/10); candidates c + (5 d2 - 2 d1)/6, c + (d2 + 2 d3)/6, c + (4 d3 - d4)/6
-    const double S = fma(WCV(W_03), E01, fma(WCV(W_06), E02, WCV(W_01) * E12));
-    const double X = WCV(W_02) * d3;  // shared by Q1 and Q2
-    const double Q0 = fma(WCV(W_5_60), d2, WCV(W_M2_60) * d1);
-    const double Q1 = fma(WCV(W_01), d2, X);
-    const double Q2 = fma(WCV(W_M005), d4, X);
-    const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
-    L = fma(num, frcp(S), c);
+  // E_jk: the weight of stencil r multiplied through by the product of all three denominators
+  //   JS: a_r = d_r/(beta_r+eps)^2                  ->  d_r (b_j b_k)^2
+  //   Z  (q = 1): a_r = d_r (1 + tau/(beta_r+eps)) = d_r (b_r + tau4)/b_r  ->  d_r (b_r + tau4) b_j b_k,
+  //      tau4 = |b0 - b2| = 4 tau (eps cancels in the difference)
+  //   M: the JS weights, normalised, then Henrick's map (below)
+  double E12, E02, E01;
+  if (WV == WENO_Z) {
+    const double tau = fabs(b0 - b2);
+    const double p12 = b1 * b2, p02 = b0 * b2, p01 = b0 * b1;
+    const double P = b0 * p12;
+    E12 = fma(tau, p12, P);
+    E02 = fma(tau, p02, P);
+    E01 = fma(tau, p01, P);
+  } else {
+    const double e0 = b0 * b0, e1 = b1 * b1, e2 = b2 * b2;
+    E12 = e1 * e2, E02 = e0 * e2, E01 = e0 * e1;
   }
-  {  // mirror image: ideal weights (3/10, 6/10, 1/10); c + (d1 - 4 d2)/6, c - (2 d2 + d3)/6, c + (2 d4 - 5 d3)/6
-    const double S = fma(WCV(W_01), E01, fma(WCV(W_06), E02, WCV(W_03) * E12));
-    const double Y = WCV(W_M02) * d2;  // shared by Q0 and Q1
-    const double Q0 = fma(WCV(W_005), d1, Y);
-    const double Q1 = fma(WCV(W_M01), d3, Y);
-    const double Q2 = fma(WCV(W_2_60), d4, WCV(W_M5_60) * d3);
-    const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
-    R = fma(num, frcp(S), c);
+  if (WV != WENO_M) {
+    {  // ideal weights (1/10, 6/10, 3/10); candidates c + (5 d2 - 2 d1)/6, c + (d2 + 2 d3)/6, c + (4 d3 - d4)/6
+      const double S = fma(WCV(W_03), E01, fma(WCV(W_06), E02, WCV(W_01) * E12));
+      const double X = WCV(W_02) * d3;  // shared by Q1 and Q2
+      const double Q0 = fma(WCV(W_5_60), d2, WCV(W_M2_60) * d1);
+      const double Q1 = fma(WCV(W_01), d2, X);
+      const double Q2 = fma(WCV(W_M005), d4, X);
+      const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
+      L = fma(num, frcp(S), c);
+    }
+    {  // mirror image: ideal weights (3/10, 6/10, 1/10); c + (d1 - 4 d2)/6, c - (2 d2 + d3)/6, c + (2 d4 - 5 d3)/6
+      const double S = fma(WCV(W_01), E01, fma(WCV(W_06), E02, WCV(W_03) * E12));
+      const double Y = WCV(W_M02) * d2;  // shared by Q0 and Q1
+      const double Q0 = fma(WCV(W_005), d1, Y);
+      const double Q1 = fma(WCV(W_M01), d3, Y);
+      const double Q2 = fma(WCV(W_2_60), d4, WCV(W_M5_60) * d3);
+      const double num = fma(E01, Q2, fma(E02, Q1, E12 * Q0));
+      R = fma(num, frcp(S), c);
+    }
+  } else {
+    // Henrick's map g_r(w) = w (d_r + d_r^2 - 3 d_r w + w^2)/(d_r^2 + w (1 - 2 d_r)) = n_r/m_r of the normalised JS weights
+    // w_r, then omega_r = g_r / sum g.  Multiplied through by m_0 m_1 m_2: A_r = n_r m_j m_k, one more reciprocal.
+    // The candidate deviations are P_r = (.)/6 with the 1/6 folded into the constants.
+    constexpr double C16 = 1.0 / 6.0, C26 = 2.0 / 6.0, C46 = 4.0 / 6.0, C56 = 5.0 / 6.0;
+    auto mapped = [&](double dA, double dB, double dC, double P0, double P1, double P2) {
+      // dA, dB, dC: ideal weights of stencils 0, 1, 2
+      const double a0 = dA * E12, a1 = dB * E02, a2 = dC * E01;
+      const double inv = frcp((a0 + a1) + a2);
+      const double w0 = a0 * inv, w1 = a1 * inv, w2 = a2 * inv;
+      const double n0 = w0 * fma(w0, w0 - 3.0 * dA, dA + dA * dA);
+      const double n1 = w1 * fma(w1, w1 - 3.0 * dB, dB + dB * dB);
+      const double n2 = w2 * fma(w2, w2 - 3.0 * dC, dC + dC * dC);
+      const double m0 = fma(w0, 1.0 - 2.0 * dA, dA * dA);
+      const double m1 = fma(w1, 1.0 - 2.0 * dB, dB * dB);
+      const double m2 = fma(w2, 1.0 - 2.0 * dC, dC * dC);
+      const double A0 = n0 * (m1 * m2), A1 = n1 * (m0 * m2), A2 = n2 * (m0 * m1);
+      const double num = fma(A2, P2, fma(A1, P1, A0 * P0));
+      return fma(num, frcp((A0 + A1) + A2), c);
+    };
+    L = mapped(0.1, 0.6, 0.3, fma(C56, d2, -C26 * d1), fma(C16, d2, C26 * d3), fma(C46, d3, -C16 * d4));
+    R = mapped(0.3, 0.6, 0.1, fma(-C46, d2, C16 * d1), fma(-C26, d2, -C16 * d3), fma(C26, d4, -C56 * d3));
   }
 }
 
+template <int WV>
 __device__ __forceinline__ void weno5(double a, double b, double c, double d, double e, double eps4, double& L,
                                       double& R) {
   const double d1 = b - a, d2 = c - b, d3 = d - c, d4 = e - d;
-  weno5_core(c, d1, d2, d3, d4, weno5_u(d2 - d1, eps4), weno5_u(d3 - d2, eps4), weno5_u(d4 - d3, eps4), L, R);
+  weno5_core<WV>(c, d1, d2, d3, d4, weno5_u(d2 - d1, eps4), weno5_u(d3 - d2, eps4), weno5_u(d4 - d3, eps4), L, R);
 }
 
 // O4 (S_L,S_R 653-654; S* 664; rho* 668; A5-A8): HLLC at one face with normal direction

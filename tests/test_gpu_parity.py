@@ -3,6 +3,8 @@ seeded inputs.  Bars (BASELINE.json north_star): relative 1e-12 i
 variable group for one RHS evaluation, 1e-9 for the state after 100 RK3 steps; bit-exact for
 mfc_prim_from_cons, the RK stage/clamp arithmetic on identical inputs, and mfc_cfl_dt.
 All tests here need a B200 (pytest -m gpu)."""
+from dataclasses import replace
+
 import numpy as np
 import pytest
 
@@ -375,3 +377,130 @@ def test_argument_errors(torch, mfc):
         mfc.Grid(2, (8, 8, 2), (1, 1, 1), (1.4,), (0.0,), (0,) * 3, (0,) * 3)
     with pytest.raises(mfc.MfcError):
         mfc.Grid(1, (8, 1, 1), (1, 1, 1), (1.4,), (0.0,), (0, 0, 0), (1, 0, 0))
+
+
+# ------------------------------------------------------------------ unit entry points, one device function at a time
+WENO_NAMES = {"js": O.RECON_WENO5, "m": O.RECON_WENO5_M, "z": O.RECON_WENO5_Z}
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("weno", ["js", "m", "z"])
+def test_weno5_values_unit_entry_point(torch, mfc, weno):
+    # mfc_weno5_values against the oracle's routine, stencil by stencil: smooth, rough, stepped and constant data over
+    # 12 decades of magnitude; error relative to the stencil's largest value
+    rng = np.random.default_rng(21)
+    n = 4096
+    s = rng.normal(size=(n, 5)) * 10.0 ** rng.integers(-3, 9, size=(n, 1))
+    s[:512] = np.sin(np.arange(5) * 0.1 + rng.uniform(0, 6, (512, 1))) * 3 + 7          # smooth
+    s[512:1024, 3:] += 1e3                                                                  # a step inside the stencil
+    s[1024:1100] = rng.normal(size=(76, 1))                                                 # constant stencils
+    case = replace(make_case(1, 1, (8, 1, 1), W.BC_EXTRAP), weno=weno)
+    g = mfc.Grid.from_case(case)
+    sd = torch.from_numpy(s.reshape(-1).copy()).cuda()
+    ld, rd = torch.empty(n, dtype=torch.float64, device="cuda"), torch.empty(n, dtype=torch.float64, device="cuda")
+    g.weno5_values(sd, ld, rd)
+    g.check()
+    got_l, got_r = ld.cpu().numpy(), rd.cpu().numpy()
+    worst = 0.0
+    for i in range(n):
+        l, r = O.weno5(WENO_NAMES[weno], s[i], case.weno_eps)
+        scale = np.abs(s[i]).max()
+        worst = max(worst, abs(got_l[i] - l) / scale, abs(got_r[i] - r) / scale)
+    g.close()
+    assert worst <= 1e-14, worst
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("ndim,nfluids", [(1, 1), (2, 2), (3, 2), (3, 3)])
+def test_hllc_faces_unit_entry_point(torch, mfc, ndim, nfluids):
+    # mfc_hllc_faces against the oracle's face solver on random admissible left/right states in every direction,
+    # including supersonic faces of both signs; error relative to the largest flux of the variable's group
+    case = make_case(ndim, nfluids, (8, 8, 8), W.BC_EXTRAP)
+    neq = case.neq
+    rng = np.random.default_rng(17)
+    n = 2000
+    rho0 = np.array([1.0, 1000.0, 0.138])[:nfluids]
+
+    def side():
+        a = rng.uniform(0.05, 1.0, (n, nfluids))
+        a /= a.sum(axis=1, keepdims=True)
+        w = np.empty((n, neq))
+        w[:, :nfluids] = a * rho0 * rng.uniform(0.8, 1.2, (n, nfluids))
+        w[:, nfluids:nfluids + ndim] = rng.uniform(-1, 1, (n, ndim)) * 10.0 ** rng.uniform(0, 3.7, (n, 1))
+        w[:, nfluids + ndim] = 10.0 ** rng.uniform(4, 9, n)
+        w[:, nfluids + ndim + 1:] = a
+        return w
+
+    wL, wR = side(), side()
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    wLd, wRd = torch.from_numpy(wL.reshape(-1).copy()).cuda(), torch.from_numpy(wR.reshape(-1).copy()).cuda()
+    for d in range(ndim):
+        Fd = torch.empty(n * neq, dtype=torch.float64, device="cuda")
+        ud = torch.empty(n, dtype=torch.float64, device="cuda")
+        g.hllc_faces(d, wLd, wRd, Fd, ud)
+        g.check()
+        F, uf = Fd.cpu().numpy().reshape(n, neq), ud.cpu().numpy()
+        Fr, ur = np.empty((n, neq)), np.empty(n)
+        for i in range(n):
+            Fr[i], ur[i], bad = orc.hllc_face(d, wL[i], wR[i])
+            assert bad == 0
+        # the measure of DESIGN.md §7: max-norm per variable group (here over the sample of faces)
+        groups = [slice(0, nfluids), slice(nfluids, nfluids + ndim), slice(nfluids + ndim, nfluids + ndim + 1),
+                  slice(nfluids + ndim + 1, neq)]
+        worst = max(np.abs(F[:, sl] - Fr[:, sl]).max() / np.abs(Fr[:, sl]).max() for sl in groups)
+        worst = max(worst, np.abs(uf - ur).max() / np.abs(ur).max())
+        # and face by face against the face's own largest flux of the group, one decade looser (cancellation between
+        # rho u^2 + p and the star correction inside one face)
+        per_face = max((np.abs(F[:, sl] - Fr[:, sl]).max(axis=1) / np.abs(Fr[:, sl]).max(axis=1)).max() for sl in groups)
+        assert per_face <= 1e-11, (d, per_face)
+        assert worst <= 1e-12, (d, worst)
+    g.close()
+
+
+# ------------------------------------------------------------------ WENO-M / WENO-Z through the whole path
+@pytest.mark.gpu
+@pytest.mark.parametrize("weno", ["m", "z"])
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_EXTRAP])
+@pytest.mark.parametrize("ndim,nfluids,n", [(1, 2, (97, 1, 1)), (2, 2, (67, 35, 1)), (3, 2, (33, 18, 11)), (3, 3, (40, 9, 13)),
+                                            (3, 1, (16, 16, 16)), (3, 2, (2, 2, 2))])
+def test_rhs_rough_state_variant_weights(torch, mfc, ndim, nfluids, n, bc, weno):
+    case = replace(make_case(ndim, nfluids, n, bc), weno=weno)
+    q = rough_state(case, 5 + ndim)
+    ref, noise = oracle_rhs_with_noise(case, q)
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None)
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("weno", ["m", "z"])
+@pytest.mark.parametrize("index,n", [(1, None), (2, None), (3, 128), (4, 48), (5, 40)])
+def test_rhs_configs_variant_weights(torch, mfc, index, n, weno):
+    case = replace(W.config(index, n=n), weno=weno)
+    q = W.initial_state(case)
+    ref, noise = oracle_rhs_with_noise(case, q)
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim, None if index in (2, 4) else noise)  # as in test_rhs_configs
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("weno", ["m", "z"])
+@pytest.mark.parametrize("index,n,nsteps", [(1, None, 100), (2, None, 100), (3, 96, 100), (4, 40, 50), (5, 32, 20)])
+def test_rk3_steps_configs_variant_weights(torch, mfc, index, n, nsteps, weno):
+    case = replace(W.config(index, n=n), weno=weno)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    for s in range(nsteps):
+        dt_ref = orc.cfl_dt(ref, case.cfl)
+        orc.rk3_step(ref, dt_ref)
+        assert orc.bad == 0
+        g.rk3_step(qd, dt_ref)
+    g.check()
+    worst, per = rel_err(qd.cpu().numpy(), ref, case.nfluids, case.ndim)
+    g.close()
+    assert worst <= STEP_TOL, per
