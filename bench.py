@@ -19,6 +19,7 @@ DESIGN.md §9) — no data-path collective; time is the max over ranks, value th
 same workload; rank 0 only.
 """
 import argparse
+import dataclasses
 import json
 import os
 import subprocess
@@ -36,6 +37,10 @@ UNIT = "ns/cell/eqn/rhs_eval"
 # each), counted by the operation-counting instantiation of the oracle and extrapolated to n -> infinity
 # (tests/test_host_logic.py re-derives them).  Key: BASELINE.json config index.
 ALG_FLOPS_PER_CELL_RHS = {1: 538.0, 2: 779.0, 3: 1798.0, 4: 3057.0, 5: 3780.0}
+# the same count with the other nonlinear weights (--weno m: mapped; --weno z: WENO-Z)
+ALG_FLOPS_PER_CELL_RHS_BY_WENO = {"js": ALG_FLOPS_PER_CELL_RHS,
+                                  "m": {1: 914.0, 2: 1343.0, 3: 3114.0, 4: 5313.0, 5: 6600.0},
+                                  "z": {1: 547.0, 2: 797.0, 3: 1844.6, 4: 3128.9, 5: 3867.6}}
 # FP64 peak "derived from unit counts and clocks": 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz.
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 # DFMA-chain microbenchmark on this pool's B200: 17.05e12 DFMA/s = 34.1 TFLOP/s (SM clock ~1.80 GHz under FP64 load)
@@ -138,7 +143,7 @@ def run_reference(args, rank):
     import mfc_workloads as W
     from oracle import oracle as O
     n_ref = {1: None, 2: None, 3: 256, 4: 64, 5: 56}[args.config]
-    case = W.config(args.config, n=n_ref)
+    case = dataclasses.replace(W.config(args.config, n=n_ref), weno=args.weno)
     q = W.initial_state(case)
     orc = O.Oracle(case)
     dt = orc.cfl_dt(q, case.cfl)
@@ -162,11 +167,11 @@ def run_reference(args, rank):
     }))
 
 
-def cpu_baseline(config_index, budget_s=20.0):
+def cpu_baseline(config_index, weno="js", budget_s=20.0):
     import mfc_workloads as W
     from oracle import oracle as O
     n_ref = {1: None, 2: None, 3: 512, 4: 128, 5: 96}[config_index]
-    case = W.config(config_index, n=n_ref)
+    case = dataclasses.replace(W.config(config_index, n=n_ref), weno=weno)
     q = W.initial_state(case)
     orc = O.Oracle(case)
     dt = orc.cfl_dt(q, case.cfl)
@@ -191,6 +196,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--n", type=int, default=None, help="override cells per direction (tests only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--weno", default="js", choices=["js", "m", "z"],
+                    help="nonlinear weights: js = BASELINE.json's WENO5-JS (default), m = mapped (the paper's default), z = WENO-Z")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -214,7 +221,7 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    case = W.config(args.config, n=args.n)
+    case = dataclasses.replace(W.config(args.config, n=args.n), weno=args.weno)
     q0 = W.initial_state(case)
     g = M.Grid.from_case(case, device=local_rank)
     qd = torch.from_numpy(q0).cuda()
@@ -257,7 +264,7 @@ def main():
     sweeps = [k for k in ("sweep_x", "sweep_y", "sweep_z") if k in kern]
     dom = max(sweeps, key=lambda k: kern[k]["ms_per_launch"] * kern[k]["launches_per_step"])
     dur_s = kern[dom]["ms_per_launch"] * 1e-3
-    flops_launch = ALG_FLOPS_PER_CELL_RHS[args.config] / case.ndim * cells
+    flops_launch = ALG_FLOPS_PER_CELL_RHS_BY_WENO[args.weno][args.config] / case.ndim * cells
     bytes_launch = sweep_alg_bytes_per_cell(dom, neq, case.ndim) * cells
     hbm_peak, hbm_src = measured_peaks()
     traffic = None
@@ -300,7 +307,7 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": case.name, "grid": list(case.n[:case.ndim]), "cells": cells, "neq": neq, "nfluids": case.nfluids,
-                   "rhs_evals_per_step": 3, "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "weno": {"js": "WENO5-JS", "m": "WENO5-M (mapped)", "z": "WENO5-Z"}[args.weno], "rhs_evals_per_step": 3, "parallelism": "replicas only" if world > 1 else "single GPU",
                    "l2": "inputs larger than L2 (state array %.0f MB vs 126 MB L2)" % (8e-6 * neq * cells) if 8 * neq * cells > 3e8
                    else "working set fits L2: latency/L2-bound configuration, roofline target does not apply"},
         "cell_updates_per_s": cells * world * args.steps / (ms * 1e-3),
@@ -308,7 +315,7 @@ def main():
         "paper_context": "PAPER.md:720-726 Table 1 (other hardware, whole step): GH200 0.32, H100 SXM 0.38, A100 0.62 ns",
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.config)
+        out["cpu_baseline"] = cpu_baseline(args.config, args.weno)
     if rank == 0:
         print(json.dumps(out))
     g.close()

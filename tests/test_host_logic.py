@@ -3,6 +3,7 @@ include/mfc_b200.h declares (no compute call — there is no GPU here), bench.py
 algorithmic flop counts its roofline line uses (re-derived with the operation-counting oracle), and the N > 1
 launch path (world_size 2, gloo)."""
 import ctypes
+import dataclasses
 import json
 import os
 import re
@@ -84,20 +85,21 @@ def test_grind_time_arithmetic():
     assert bench.FP64_PEAK_TFLOPS_DERIVED == pytest.approx(37.225, rel=1e-3)
 
 
+@pytest.mark.parametrize("weno", ["js", "m", "z"])
 @pytest.mark.parametrize("index,n", [(1, 400), (2, 400), (3, 48), (4, 16), (5, 16)])
-def test_algorithmic_flops_per_cell_match_the_operation_counting_oracle(index, n):
+def test_algorithmic_flops_per_cell_match_the_operation_counting_oracle(index, n, weno):
     """bench.ALG_FLOPS_PER_CELL_RHS is the n -> infinity value of (add + mul + div + sqrt)/cells.  One face more
     than cells per line is solved, so the count on n cells per direction is  A + B/n  exactly; two sizes fix A."""
     import bench
 
     def per_cell(m):
-        case = W.config(index, n=m)
+        case = dataclasses.replace(W.config(index, n=m), weno=weno)
         c = O.Oracle(case).count_rhs(W.initial_state(case))
         return (c["add"] + c["mul"] + c["div"] + c["sqrt"]) / case.cells
 
     f1, f2 = per_cell(n), per_cell(2 * n)
     a = 2 * f2 - f1  # f(n) = A + B/n
-    assert a == pytest.approx(bench.ALG_FLOPS_PER_CELL_RHS[index], rel=2e-3), (f1, f2, a)
+    assert a == pytest.approx(bench.ALG_FLOPS_PER_CELL_RHS_BY_WENO[weno][index], rel=2e-3), (f1, f2, a)
 
 
 def test_reference_arm_prints_the_contract_line():
