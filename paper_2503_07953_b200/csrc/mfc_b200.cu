@@ -721,6 +721,9 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, doubl
     if (!attr_done[g->device & 15]) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       if (e != cudaSuccess) return e;
+      // the rings want all of the SM's shared memory (two blocks of up to 113 KB); the sweeps make no use of L1
+      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+      if (e != cudaSuccess) return e;
       attr_done[g->device & 15] = true;
     }
     Scope sc(g, DIR == 1 ? MFC_K_SWEEP_Y : MFC_K_SWEEP_Z);
