@@ -41,6 +41,7 @@ class Case:
     t_end: float = 0.0
     seed: int = DEFAULT_SEED
     builder: str = ""        # which generator below makes q0
+    model: str = "allaire"   # volume-fraction equation: "allaire" (no K div u) or "kapila" (eq. 5; two fluids)
     weno: str = "js"         # nonlinear weights: "js" (BASELINE.json), "m" (mapped), "z"
 
     @property

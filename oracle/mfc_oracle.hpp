@@ -39,6 +39,9 @@ constexpr int kMaxEq = 2 * kMaxFluids + 3 + 1;
 enum { BC_PERIODIC = 0, BC_EXTRAP = 1 };
 // RECON_WENO5_M: mapped weights of Henrick et al. (the paper's ref. [30]);
 // RECON_WENO5_Z: WENO-Z weights (§4.2.2) with q = 1.
+// MODEL_ALLAIRE: d(alpha_i)/dt + u.grad(alpha_i) = 0 ("the model reduces to that of Allaire et al.");
+// MODEL_KAPILA: ... = K_i div(u) with eq.(5), two fluids.
+enum { MODEL_ALLAIRE = 0, MODEL_KAPILA = 1 };
 enum { RECON_PIECEWISE_CONSTANT = 1, RECON_WENO5_JS = 5, RECON_WENO5_M = 6, RECON_WENO5_Z = 7 };
 
 // generic helpers so that T may be double, long double or the counting type
@@ -62,6 +65,7 @@ struct Params {
   T alpha_floor = T(1e-6); // A10
   int clamp = 0;           // A10
   int recon = RECON_WENO5_JS;
+  int model = MODEL_ALLAIRE;
 
   int neq() const { return 2 * nfluids + ndim + 1; }  // PAPER.md:704 "two advected species (8 PDEs)" in 3D
   std::size_t cells() const { return std::size_t(n[0]) * n[1] * n[2]; }
@@ -123,6 +127,19 @@ int prim_from_cons_cell(const Params<T>& P, const T* q, T* w) {
 template <class T>
 T sound_speed_sq(const T& Gam, const T& Pi, const T& p, const T& rho) {
   return ((Gam + T(1)) * p + Pi) / (Gam * rho);
+}
+
+// O5-K (eqs.(5),(6)): the coefficient K of the K div(u) term of the alpha_1 equation for two
+// fluids, from the cell's pressure and volume fractions.  With rho_i c_i^2 = gamma_i (p + pi_inf_i) (eq. 6)
+//   K = (rho_2 c_2^2 - rho_1 c_1^2) / (rho_1 c_1^2/alpha_1 + rho_2 c_2^2/alpha_2).
+// The paper prints a "+" in the numerator; it must be "-" (reading A13): that is what
+// isentropic compression of each phase at common pressure gives (pinned in tests/test_oracle_kapila.py), and
+// only then does K vanish for two identical fluids.  The alpha_2 equation takes -K, so that sum alpha_i stays 1.
+template <class T>
+T kapila_K(const Params<T>& P, const T& p, const T& alpha1, const T& alpha2) {
+  const T A1 = P.gamma[0] * (p + P.pi_inf[0]);
+  const T A2 = P.gamma[1] * (p + P.pi_inf[1]);
+  return (A2 - A1) / (A1 / alpha1 + A2 / alpha2);
 }
 
 // O3 (Jiang-Shu coefficients of the paper's refs [30],[70], A3).
@@ -390,6 +407,13 @@ struct Solver {
           for (int f = 0; f < N; ++f) {
             std::size_t t = idx(P.i_alpha(f), ijk[0], ijk[1], ijk[2]);
             rhs_out[t] = rhs_out[t] + q[t] * (uf[i + 1] - uf[i]) / P.dx[dir];
+          }
+          if (P.model == MODEL_KAPILA && N == 2) {  // K div(u), direction by direction, cell-centre K
+            const T* wc = &wl[std::size_t(i + 3) * neq];
+            const T K = kapila_K(P, wc[P.i_E()], wc[P.i_alpha(0)], wc[P.i_alpha(1)]);
+            std::size_t t1 = idx(P.i_alpha(0), ijk[0], ijk[1], ijk[2]), t2 = idx(P.i_alpha(1), ijk[0], ijk[1], ijk[2]);
+            rhs_out[t1] = rhs_out[t1] + K * (uf[i + 1] - uf[i]) / P.dx[dir];
+            rhs_out[t2] = rhs_out[t2] - K * (uf[i + 1] - uf[i]) / P.dx[dir];
           }
         }
       }

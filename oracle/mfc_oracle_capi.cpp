@@ -26,6 +26,7 @@ typedef struct {
   double alpha_floor;
   int clamp;
   int recon;
+  int model;
 } oracle_params;
 
 }  // extern "C"
@@ -51,6 +52,7 @@ Params<T> convert(const oracle_params* p) {
   P.alpha_floor = T(p->alpha_floor);
   P.clamp = p->clamp;
   P.recon = p->recon;
+  P.model = p->model;
   P.derive();
   return P;
 }
@@ -138,6 +140,10 @@ void oracle_weno5_ld(int recon, const double* s, double eps, double* left, doubl
 // the weights step alone: omega[3] from ideal weights dr[3] and smoothness indicators beta[3]
 void oracle_weno5_weights(int recon, const double* dr, const double* beta, double eps, double* omega) {
   weno5_weights<double>(recon, dr, beta, eps, omega);
+}
+
+double oracle_kapila_K(const oracle_params* p, double pres, double alpha1, double alpha2) {
+  return kapila_K<double>(convert<double>(p), pres, alpha1, alpha2);
 }
 
 int oracle_hllc_face(const oracle_params* p, int dir, const double* wL, const double* wR, double* F, double* uf) {

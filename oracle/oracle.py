@@ -14,6 +14,7 @@ from . import build as _build
 BC_PERIODIC, BC_EXTRAP = 0, 1
 RECON_PC, RECON_WENO5 = 1, 5
 RECON_WENO5_M, RECON_WENO5_Z = 6, 7   # mapped (Henrick) and WENO-Z weights
+MODEL_BY_NAME = {"allaire": 0, "kapila": 1}   # PAPER.md:86 / 59, 78-86
 RECON_BY_NAME = {"js": RECON_WENO5, "m": RECON_WENO5_M, "z": RECON_WENO5_Z}
 _MAXF = 4
 
@@ -22,7 +23,7 @@ class OracleParams(C.Structure):
     _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("dx", C.c_double * 3), ("nfluids", C.c_int),
                 ("gamma", C.c_double * _MAXF), ("pi_inf", C.c_double * _MAXF),
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
-                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("recon", C.c_int)]
+                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("recon", C.c_int), ("model", C.c_int)]
 
 
 _lib = None
@@ -46,6 +47,8 @@ def lib():
         L.oracle_weno5_js_ld.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js_ld.restype = None
         L.oracle_weno5.argtypes = [C.c_int, dp, C.c_double, dp, dp]; L.oracle_weno5.restype = None
         L.oracle_weno5_ld.argtypes = [C.c_int, dp, C.c_double, dp, dp]; L.oracle_weno5_ld.restype = None
+        L.oracle_kapila_K.argtypes = [C.POINTER(OracleParams), C.c_double, C.c_double, C.c_double]
+        L.oracle_kapila_K.restype = C.c_double
         L.oracle_weno5_weights.argtypes = [C.c_int, dp, dp, C.c_double, dp]; L.oracle_weno5_weights.restype = None
         L.oracle_hllc_face.argtypes = [pp, C.c_int, dp, dp, dp, dp]
         L.oracle_clamp_cell.argtypes = [pp, dp]; L.oracle_clamp_cell.restype = None
@@ -80,6 +83,7 @@ def make_params(case, recon=None):
     p.alpha_floor = case.alpha_floor
     p.clamp = int(case.clamp)
     p.recon = recon
+    p.model = MODEL_BY_NAME[getattr(case, "model", "allaire")]
     return p
 
 
@@ -131,6 +135,9 @@ class Oracle:
         uf = C.c_double()
         bad = lib().oracle_hllc_face(C.byref(self.p), d, _dp(wL), _dp(wR), _dp(F), C.byref(uf))
         return F, uf.value, bad
+
+    def kapila_K(self, p, alpha1, alpha2):
+        return lib().oracle_kapila_K(C.byref(self.p), float(p), float(alpha1), float(alpha2))
 
     def clamp_cell(self, q):
         q = np.ascontiguousarray(q, dtype=np.float64).copy()
