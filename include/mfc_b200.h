@@ -63,6 +63,12 @@ typedef enum { MFC_BC_PERIODIC = 0, MFC_BC_EXTRAP = 1 } mfc_bc;
  * tau = |beta_0 - beta_2| (PAPER.md:562-566 with q = 1). */
 typedef enum { MFC_WENO_JS = 0, MFC_WENO_M = 1, MFC_WENO_Z = 2 } mfc_weno;
 
+/* Volume-fraction equation: d(alpha_i)/dt + u.grad(alpha_i) = K_i div(u).  ALLAIRE: K_i = 0 ("for some
+ * problems K div(u) is not necessary, and the model reduces to that of Allaire et al.", PAPER.md:86 — what
+ * BASELINE.json names).  KAPILA: two fluids, K_1 = K of eq. (5) (numerator rho_2 c_2^2 - rho_1 c_1^2),
+ * K_2 = -K, with the cell-centre p and alpha_i and the face velocities of the Riemann solver. */
+typedef enum { MFC_MODEL_ALLAIRE = 0, MFC_MODEL_KAPILA = 1 } mfc_model;
+
 #define MFC_MAX_FLUIDS 3
 
 typedef struct {
@@ -77,6 +83,7 @@ typedef struct {
   double alpha_floor;    /* volume-fraction floor of the RK-stage clamp (A10) */
   int clamp;             /* 0: no clamp; 1: apply A10 after every RK stage */
   int weno;              /* mfc_weno: nonlinear weights of the reconstruction; 0 = MFC_WENO_JS */
+  int model;             /* mfc_model: 0 = MFC_MODEL_ALLAIRE; MFC_MODEL_KAPILA needs nfluids == 2 */
   int device;            /* CUDA device ordinal */
   void *stream;          /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
 } mfc_params;

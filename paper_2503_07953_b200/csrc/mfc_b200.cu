@@ -25,6 +25,9 @@
 namespace mfc {
 
 constexpr unsigned FULL = 0xffffffffu;
+// The template parameter WV of the sweeps encodes the nonlinear weights (WV % 3: WENO_JS / WENO_M / WENO_Z) and the
+// volume-fraction model (WV / 3: 0 Allaire, 1 Kapila) — both compile-time, so that neither costs the other anything.
+#define KAPILA_ON(kp) (WV >= 3)
 // Tuning knobs (compile-time; the defaults are the measured best on B200).
 #ifndef MFC_XW
 #define MFC_XW 4          // warps per block, sweep_x
@@ -207,7 +210,7 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
     double WL[NEQ], WR[NEQ];
 #pragma unroll
     for (int v = 0; v < NEQ; ++v)
-      weno5<WV>(rg[v][Q & 63], rg[v][(Q + 1) & 63], rg[v][(Q + 2) & 63], rg[v][(Q + 3) & 63], rg[v][(Q + 4) & 63],
+      weno5<WV % 3>(rg[v][Q & 63], rg[v][(Q + 1) & 63], rg[v][(Q + 2) & 63], rg[v][(Q + 3) & 63], rg[v][(Q + 4) & 63],
             kp.eps4, WL[v], WR[v]);
     // left neighbour's value by a rotate: lane 31 sends what it had in the previous step
     double WLf[NEQ];
@@ -235,7 +238,15 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
       for (int v = 0; v < NEQ; ++v) {
         r[v] = (Fm[v] - F[v]) * idx;
         if (v >= IA) r[v] = fma(rg[v][(Q + 1) & 63], du, r[v]);
-        if (ACCUM) r[v] += rhs[v * kp.ncells + off];
+      }
+      if (N == 2 && KAPILA_ON(kp)) {  // K div(u), this direction's part (eq. 5)
+        const double Kdu = kapila_K(kp, rg[N + D][(Q + 1) & 63], rg[IA][(Q + 1) & 63], rg[IA + 1][(Q + 1) & 63]) * du;
+        r[IA] += Kdu;
+        r[IA + 1] -= Kdu;
+      }
+      if (ACCUM) {
+#pragma unroll
+        for (int v = 0; v < NEQ; ++v) r[v] += rhs[v * kp.ncells + off];
       }
       if (STAGE >= 1) {
         double qnc[NEQ], qsc[NEQ];
@@ -396,6 +407,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
     double am[N];  // alpha_i of cell g-1 (source term of its update), read before its slot is reused
 #pragma unroll
     for (int i = 0; i < N; ++i) am[i] = *elem(i0, IA + i);
+    const double pm = (N == 2 && KAPILA_ON(kp)) ? *elem(i0, N + D) : 0.0;  // its pressure, for K (Kapila model only)
     double w[NEQ];
     bad |= prim_cell<N, D, false>(kp, qn, w);  // cell g+2
     {  // prefetch of cell s0+3+p, branch-free (in the last step, p = L+1, the value is not used; any valid cell will do)
@@ -432,8 +444,8 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
       st2(i0, h, make_double2(w[2 * h], two ? w[two ? 2 * h + 1 : 0] : 0.0));
       st2(S_D * SLOT + i0, h, d4);
       st2(S_U * SLOT + j0, h, u2);
-      weno5_core<WV>(c.x, d1.x, d2.x, d3.x, d4.x, u0.x, u1.x, u2.x, WL[2 * h], WR[2 * h]);
-      if (two) weno5_core<WV>(c.y, d1.y, d2.y, d3.y, d4.y, u0.y, u1.y, u2.y, WL[two ? 2 * h + 1 : 0], WR[two ? 2 * h + 1 : 0]);
+      weno5_core<WV % 3>(c.x, d1.x, d2.x, d3.x, d4.x, u0.x, u1.x, u2.x, WL[2 * h], WR[2 * h]);
+      if (two) weno5_core<WV % 3>(c.y, d1.y, d2.y, d3.y, d4.y, u0.y, u1.y, u2.y, WL[two ? 2 * h + 1 : 0], WR[two ? 2 * h + 1 : 0]);
     }
     {
       const int t = i0;
@@ -451,6 +463,11 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
       for (int v = 0; v < NEQ; ++v) {
         r[v] = (Fp[v] - F[v]) * idx;
         if (v >= IA) r[v] = fma(am[v - IA], du, r[v]);
+      }
+      if (N == 2 && KAPILA_ON(kp)) {  // K div(u), this direction's part (eq. 5)
+        const double Kdu = kapila_K(kp, pm, am[0], am[N - 1]) * du;
+        r[IA] += Kdu;
+        r[IA + 1] -= Kdu;
       }
       if (ACCUM || STAGE >= 1) cp_async_wait_all();
       if (ACCUM) {
@@ -721,9 +738,6 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, doubl
     if (!attr_done[g->device & 15]) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       if (e != cudaSuccess) return e;
-      // the rings want all of the SM's shared memory (two blocks of up to 113 KB); the sweeps make no use of L1
-      e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-      if (e != cudaSuccess) return e;
       attr_done[g->device & 15] = true;
     }
     Scope sc(g, DIR == 1 ? MFC_K_SWEEP_Y : MFC_K_SWEEP_Z);
@@ -767,6 +781,8 @@ static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* q
 // rhs = L(q) restricted to the directions in mask.  mask == all: x overwrites, y and z accumulate.
 template <int N, int D, int WV>
 static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mask) {
+  if constexpr (WV >= 3 && N != 2) return cudaErrorInvalidValue;  // Kapila: two fluids only (not instantiated otherwise)
+  else {
   const int all = (1 << D) - 1;
   cudaError_t e;
   if ((mask & all) == all) {
@@ -781,6 +797,7 @@ static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mas
   if (D >= 3 && (mask & 4))
     if ((e = launch_march<N, D, WV, 2, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   return cudaSuccess;
+  }
 }
 
 // One RK stage: L(qs) by the D sweeps, the last of which applies the stage combination and the clamp itself
@@ -807,10 +824,13 @@ static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, dou
 //   stage 3 sweeps B,  partial L in A, q^{n+1} ends in q.
 template <int N, int D, int WV>
 static cudaError_t launch_rk3(mfc_grid* g, double* q, double dt) {
-  cudaError_t e;
-  if ((e = launch_stage<N, D, WV, 1>(g, q, g->Lq, q, dt)) != cudaSuccess) return e;
-  if ((e = launch_stage<N, D, WV, 2>(g, g->Lq, g->q1, q, dt)) != cudaSuccess) return e;
-  return launch_stage<N, D, WV, 3>(g, g->q1, g->Lq, q, dt);
+  if constexpr (WV >= 3 && N != 2) return cudaErrorInvalidValue;  // Kapila: two fluids only
+  else {
+    cudaError_t e;
+    if ((e = launch_stage<N, D, WV, 1>(g, q, g->Lq, q, dt)) != cudaSuccess) return e;
+    if ((e = launch_stage<N, D, WV, 2>(g, g->Lq, g->q1, q, dt)) != cudaSuccess) return e;
+    return launch_stage<N, D, WV, 3>(g, g->q1, g->Lq, q, dt);
+  }
 }
 
 template <int N, int D>
@@ -867,17 +887,23 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
 #define MFC_DISPATCH_W(g, EXPR)                                                   \
   [&]() -> cudaError_t {                                                          \
     constexpr int WV = WENO_JS;                                                   \
-    return (g)->weno == WENO_JS ? MFC_DISPATCH(g, EXPR) : cudaErrorInvalidValue;  \
+    return (g)->weno == WENO_JS && !(g)->kp.kapila ? MFC_DISPATCH(g, EXPR) : cudaErrorInvalidValue;  \
   }()
 #else
-#define MFC_DISPATCH_W(g, EXPR)                                                   \
-  [&]() -> cudaError_t {                                                          \
-    switch ((g)->weno) {                                                          \
-      case WENO_JS: { constexpr int WV = WENO_JS; return MFC_DISPATCH(g, EXPR); } \
-      case WENO_M: { constexpr int WV = WENO_M; return MFC_DISPATCH(g, EXPR); }   \
-      case WENO_Z: { constexpr int WV = WENO_Z; return MFC_DISPATCH(g, EXPR); }   \
-    }                                                                             \
-    return cudaErrorInvalidValue;                                                 \
+#define MFC_DISPATCH_W1(g, K, EXPR)                                                          \
+  switch ((g)->weno) {                                                                           \
+    case WENO_JS: { constexpr int WV = WENO_JS + 3 * K; return MFC_DISPATCH(g, EXPR); }          \
+    case WENO_M: { constexpr int WV = WENO_M + 3 * K; return MFC_DISPATCH(g, EXPR); }            \
+    case WENO_Z: { constexpr int WV = WENO_Z + 3 * K; return MFC_DISPATCH(g, EXPR); }            \
+  }
+#define MFC_DISPATCH_W(g, EXPR)                                                                  \
+  [&]() -> cudaError_t {                                                                         \
+    if ((g)->kp.kapila) {                                                                        \
+      MFC_DISPATCH_W1(g, 1, EXPR)                                                                \
+    } else {                                                                                     \
+      MFC_DISPATCH_W1(g, 0, EXPR)                                                                \
+    }                                                                                            \
+    return cudaErrorInvalidValue;                                                                \
   }()
 #endif
 
@@ -911,6 +937,10 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   for (int i = 0; i < p->nfluids; ++i)
     if (!(p->gamma[i] > 1.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: gamma_i must be > 1");
   if (!(p->weno_eps > 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: weno_eps must be > 0");
+  if (p->model != MFC_MODEL_ALLAIRE && p->model != MFC_MODEL_KAPILA)
+    return fail(MFC_ERR_ARG, "mfc_init_grid: model must be MFC_MODEL_ALLAIRE or MFC_MODEL_KAPILA");
+  if (p->model == MFC_MODEL_KAPILA && p->nfluids != 2)
+    return fail(MFC_ERR_ARG, "mfc_init_grid: MFC_MODEL_KAPILA is defined for two fluids (PAPER.md:78, eq. 5)");
   if (p->weno != MFC_WENO_JS && p->weno != MFC_WENO_M && p->weno != MFC_WENO_Z)
     return fail(MFC_ERR_ARG, "mfc_init_grid: weno must be MFC_WENO_JS, MFC_WENO_M or MFC_WENO_Z");
   int ndev = 0;
@@ -943,6 +973,11 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   g->kp.eps4 = 4.0 * p->weno_eps;
   g->kp.alpha_floor = p->alpha_floor;
   g->kp.clamp = p->clamp ? 1 : 0;
+  g->kp.kapila = p->model == MFC_MODEL_KAPILA ? 1 : 0;
+  for (int i = 0; i < 2 && i < p->nfluids; ++i) {
+    g->kp.gam[i] = p->gamma[i];
+    g->kp.gpi[i] = p->gamma[i] * p->pi_inf[i];
+  }
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, p->device) == cudaSuccess) g->num_sms = prop.multiProcessorCount;
   default_segments(g);

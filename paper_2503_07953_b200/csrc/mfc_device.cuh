@@ -20,6 +20,9 @@ struct KP {
   double eps4;   // 4 * weno_eps (the smoothness indicators are carried scaled by 4)
   double alpha_floor;
   int clamp;
+  int kapila;    // 1: add K div(u) to the volume-fraction equations (two fluids)
+  double gam[2]; // gamma_i and gamma_i pi_inf_i of the two fluids: rho_i c_i^2 = gamma_i p + gamma_i pi_inf_i (eq. 6)
+  double gpi[2];
   int* flag;     // sticky non-physical flag (A19)
 };
 
@@ -38,6 +41,15 @@ __device__ __forceinline__ double frcp(double x) {
   const double e = fma(-x, y, 1.0);
   const double t = fma(e, e, e);
   return fma(y, t, y);
+}
+
+// O5-K (eq.(5) with the sign of reading A13): K of the alpha_1 equation for two fluids,
+//   K = (A2 - A1)/(A1/alpha_1 + A2/alpha_2) = alpha_1 alpha_2 (A2 - A1)/(alpha_2 A1 + alpha_1 A2),  A_i = rho_i c_i^2 = gamma_i (p + pi_inf_i);
+// the second form has one reciprocal and is 0, not 0/0, when a volume fraction vanishes.
+__device__ __forceinline__ double kapila_K(const KP& kp, double p, double a1, double a2) {
+  const double A1 = fma(kp.gam[0], p, kp.gpi[0]), A2 = fma(kp.gam[1], p, kp.gpi[1]);
+  const double den = fma(a2, A1, a1 * A2);
+  return ((a1 * a2) * (A2 - A1)) * frcp(den);
 }
 
 // sqrt(x) for normal x > 0: hardware rsqrt seed, one coupled (Goldschmidt) step, one residual correction.

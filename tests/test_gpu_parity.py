@@ -504,3 +504,58 @@ def test_rk3_steps_configs_variant_weights(torch, mfc, index, n, nsteps, weno):
     worst, per = rel_err(qd.cpu().numpy(), ref, case.nfluids, case.ndim)
     g.close()
     assert worst <= STEP_TOL, per
+
+
+# ------------------------------------------------------------------ Kapila model: K div(u) in the alpha equations
+@pytest.mark.gpu
+@pytest.mark.parametrize("weno", ["js", "z"])
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_EXTRAP])
+@pytest.mark.parametrize("ndim,n", [(1, (97, 1, 1)), (2, (67, 35, 1)), (3, (33, 18, 11)), (3, (2, 2, 2))])
+def test_rhs_rough_state_kapila(torch, mfc, ndim, n, bc, weno):
+    case = replace(make_case(ndim, 2, n, bc), model="kapila", weno=weno)
+    q = rough_state(case, 5 + ndim)
+    ref, _ = oracle_rhs_with_noise(case, q)
+    allaire = O.Oracle(replace(case, model="allaire")).rhs(q)
+    assert np.abs(ref - allaire)[case.nfluids + ndim + 1:].max() > 1e-3 * np.abs(ref[case.nfluids + ndim + 1:]).max()  # the term is there
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, 2, ndim)
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mask", [1, 2, 4])
+def test_rhs_single_directions_kapila(torch, mfc, mask):
+    case = replace(make_case(3, 2, (33, 18, 11), W.BC_EXTRAP), model="kapila")
+    q = rough_state(case, 3)
+    orc = O.Oracle(case)
+    ref = orc.rhs(q, dir_mask=mask)
+    got = gpu_rhs(torch, mfc, case, q, mask=mask)
+    worst, per = rel_err(got, ref, 2, 3)
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("index,n,nsteps", [(2, None, 100), (3, 96, 100), (4, 40, 50)])
+def test_rk3_steps_configs_kapila(torch, mfc, index, n, nsteps):
+    case = replace(W.config(index, n=n), model="kapila")
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    for s in range(nsteps):
+        dt_ref = orc.cfl_dt(ref, case.cfl)
+        orc.rk3_step(ref, dt_ref)
+        assert orc.bad == 0
+        g.rk3_step(qd, dt_ref)
+    g.check()
+    worst, per = rel_err(qd.cpu().numpy(), ref, case.nfluids, case.ndim)
+    g.close()
+    assert worst <= STEP_TOL, per
+
+
+@pytest.mark.gpu
+def test_kapila_needs_two_fluids(torch, mfc):
+    with pytest.raises(mfc.MfcError) as e:
+        mfc.Grid.from_case(replace(make_case(1, 3, (16, 1, 1), W.BC_EXTRAP), model="kapila"))
+    assert e.value.status == mfc.MFC_ERR_ARG

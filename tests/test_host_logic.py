@@ -136,7 +136,8 @@ def test_replica_launch_path_world_size_2_gloo(tmp_path):
                           "--master-addr", "127.0.0.1", "--master-port", "29577", str(script)],
                          capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
     assert out.returncode == 0, out.stderr[-2000:]
-    recs = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    # the two ranks write to one pipe: their lines may arrive glued together
+    recs = [json.loads(m) for m in re.findall(r"\{[^{}]*\}", out.stdout)]
     assert sorted(r["rank"] for r in recs) == [0, 1]
     for r in recs:
         assert r["ms"] == 15.0
