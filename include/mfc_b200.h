@@ -55,7 +55,10 @@ typedef enum {
 /* Ghost-cell ("buffer region") boundary conditions, PAPER.md:203 (§3.3).  Extrapolation is the paper's
  * first-order extrapolation (ghost = nearest interior cell); periodic is required by BASELINE.json
  * (the paper's Taylor-Green case, implies it).  Periodic must be set on both ends. */
-typedef enum { MFC_BC_PERIODIC = 0, MFC_BC_EXTRAP = 1 } mfc_bc;
+typedef enum { MFC_BC_PERIODIC = 0, MFC_BC_EXTRAP = 1, MFC_BC_HALO = 2 } mfc_bc;
+/* MFC_BC_HALO (slab decomposition, the paper's "buffer regions ... populated through message passing", PAPER.md:203,
+ * 762-770): allowed on either end of the LAST direction of a 2-D or 3-D grid.  The three ghost layers beyond that
+ * end are read from an array the caller fills before every RHS evaluation (mfc_set_halo). */
 
 /* Nonlinear weights of the fifth-order WENO reconstruction.  JS: alpha_r = d_r/(beta_r+eps)^2
  * (the weights BASELINE.json names).  M: the JS weights passed through the map of Henrick et al. and
@@ -121,6 +124,24 @@ mfc_status mfc_rk3_step(mfc_grid *g, double *q, double dt);
 
 /* nsteps RK3 steps with a fixed dt (one call, same arithmetic as nsteps calls of mfc_rk3_step).  async. */
 mfc_status mfc_rk3_steps(mfc_grid *g, double *q, double dt, int nsteps);
+
+/* Slab decomposition along the last direction (one handle per slab, one process per GPU).
+ * mfc_set_halo: device arrays of the ghost layers beyond the low / high end, each neq*3*plane doubles laid out
+ *   [v][layer][plane], plane = cells / n[ndim-1] in the grid's own order, layer l = 0..2 <-> logical cells -3+l (low end)
+ *   and n+l (high end).  Caller-owned, must stay valid and hold the neighbour's data whenever a sweep runs; an end
+ *   without MFC_BC_HALO may pass NULL.
+ * mfc_rk3_stage: stage s = 1, 2, 3 of the RK3 step alone (mfc_rk3_step == the three in order).  With halos the caller
+ *   refreshes them from the state the stage sweeps before each stage; mfc_stage_input returns that array
+ *   (stage 1: q itself; stages 2, 3: the handle's stage state), neq*cells doubles, device.  async.
+ * mfc_rk3_step(s), mfc_advance and the *_host calls refuse a handle with MFC_BC_HALO (they cannot refresh halos).
+ * mfc_pack_halo: copies the three layers next to the low end (cells 0..2 of the last direction) of that same array into
+ *   send_lo and the three next to the high end (cells n-3..n-1) into send_hi, both [v][layer][plane], device, either may
+ *   be NULL.  What a slab packs as send_lo is its lower neighbour's halo_hi; send_hi is the upper neighbour's halo_lo.
+ *   async on the handle's stream. */
+mfc_status mfc_set_halo(mfc_grid *g, const double *halo_lo, const double *halo_hi);
+mfc_status mfc_pack_halo(mfc_grid *g, const double *q, int stage, double *send_lo, double *send_hi);
+mfc_status mfc_rk3_stage(mfc_grid *g, double *q, double dt, int stage);
+mfc_status mfc_stage_input(mfc_grid *g, const double *q, int stage, const double **state_out);
 
 /* dt = cfl / max_cells sum_d (|u_d| + c)/dx_d  with the frozen-alpha mixture sound speed
  * c^2 = ((Gamma+1) p + Pi)/(Gamma rho)  (A5, A9; not in the paper — BASELINE.json asks for it).

@@ -10,7 +10,7 @@ import os
 
 from . import build as _build
 
-BC_PERIODIC, BC_EXTRAP = 0, 1
+BC_PERIODIC, BC_EXTRAP, BC_HALO = 0, 1, 2
 WENO_JS, WENO_M, WENO_Z = 0, 1, 2
 WENO_BY_NAME = {"js": WENO_JS, "m": WENO_M, "z": WENO_Z}
 MODEL_ALLAIRE, MODEL_KAPILA = 0, 1
@@ -19,7 +19,8 @@ MFC_OK, MFC_ERR_ARG, MFC_ERR_ALLOC, MFC_ERR_CUDA, MFC_ERR_NONPHYSICAL = 0, 1, 2,
 EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "mfc_prim_from_cons", "mfc_rhs",
            "mfc_rhs_dirs", "mfc_rk3_step", "mfc_rk3_steps", "mfc_cfl_dt", "mfc_check", "mfc_rhs_host",
            "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
-           "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error")
+           "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error", "mfc_set_halo", "mfc_rk3_stage",
+           "mfc_stage_input", "mfc_pack_halo")
 
 
 KERNEL_CLASSES = ("prim", "sweep_x", "sweep_y", "sweep_z", "rk", "cfl")
@@ -77,6 +78,10 @@ def lib():
         L.mfc_launch_count.argtypes = [vp]; L.mfc_launch_count.restype = C.c_longlong
         L.mfc_set_segments.argtypes = [vp, C.c_int, C.c_int, C.c_int]
         L.mfc_last_error.restype = C.c_char_p
+        L.mfc_set_halo.argtypes = [vp, dp, dp]
+        L.mfc_rk3_stage.argtypes = [vp, dp, C.c_double, C.c_int]
+        L.mfc_stage_input.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_void_p)]
+        L.mfc_pack_halo.argtypes = [vp, dp, C.c_int, dp, dp]
         _lib = L
     return _lib
 
@@ -225,6 +230,27 @@ class Grid:
         n = uf.numel()
         _ck(lib().mfc_hllc_faces(self._h, int(direction), _dev_ptr(wL, n * self.neq), _dev_ptr(wR, n * self.neq), n,
                                  _dev_ptr(F, n * self.neq), _dev_ptr(uf, n)))
+
+    def set_halo(self, halo_lo, halo_hi):
+        """halo_lo / halo_hi: CUDA float64 tensors of neq*3*plane elements ([v][layer][plane]) or None; kept alive here"""
+        self._halo = (halo_lo, halo_hi)
+        lo = _dev_ptr(halo_lo, halo_lo.numel()) if halo_lo is not None else None
+        hi = _dev_ptr(halo_hi, halo_hi.numel()) if halo_hi is not None else None
+        _ck(lib().mfc_set_halo(self._h, lo, hi))
+
+    def pack_halo(self, q, stage, send_lo, send_hi):
+        lo = _dev_ptr(send_lo, send_lo.numel()) if send_lo is not None else None
+        hi = _dev_ptr(send_hi, send_hi.numel()) if send_hi is not None else None
+        _ck(lib().mfc_pack_halo(self._h, _dev_ptr(q, self.count), int(stage), lo, hi))
+
+    def rk3_stage(self, q, dt, stage):
+        _ck(lib().mfc_rk3_stage(self._h, _dev_ptr(q, self.count), float(dt), int(stage)))
+
+    def stage_input_ptr(self, q, stage):
+        """device address of the array stage `stage` sweeps (stage 1: q itself)"""
+        out = C.c_void_p()
+        _ck(lib().mfc_stage_input(self._h, _dev_ptr(q, self.count), int(stage), C.byref(out)))
+        return out.value
 
     def launch_count(self):
         return lib().mfc_launch_count(self._h)

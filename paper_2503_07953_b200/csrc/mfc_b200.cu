@@ -356,6 +356,19 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
 #pragma unroll
     for (int v = 0; v < NEQ; ++v) qn[v] = __ldg(q + v * kp.ncells + off);
   };
+  // BC_HALO (last direction only): ghost layer l = 0..2 beyond an end comes from the halo array of that end,
+  // [neq][3][plane] with plane == stride; `base` is the column's offset within a plane.
+  constexpr bool HALO_DIR = DIR == D - 1;
+  auto loadh = [&](const double* halo, int layer) {
+    const double* src = halo + ((long long)layer * stride + base);
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) qn[v] = __ldg(src + (long long)v * 3 * stride);
+  };
+  auto load_cell = [&](int cell) {  // logical cell -3..n+2 through the ghost map (O1) or the halo
+    if (HALO_DIR && lo == BC_HALO && cell < 0) loadh(kp.halo_lo, cell + 3);
+    else if (HALO_DIR && hi == BC_HALO && cell >= n) loadh(kp.halo_hi, min(cell - n, 2));
+    else loadq(base + ghost_index(cell, n, lo, hi) * stride);
+  };
   // rotating slot offsets (in doubles): i0 = oldest of the 3-slot rings (w of cell g-1, d1), i2 = newest;
   // j0 = older of the 2 u slots.
   int i0 = 0, i1 = SLOT, i2 = 2 * SLOT, j0 = 0, j1 = SLOT;
@@ -365,7 +378,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
     for (int v = 0; v < NEQ; ++v) wp[v] = dp[v] = 0.0;
 #pragma unroll 1
     for (int m = 0; m < 4; ++m) {
-      loadq(base + ghost_index(s0 - 3 + m, n, lo, hi) * stride);
+      load_cell(s0 - 3 + m);
       double w[NEQ];
       bad |= prim_cell<N, D, false>(kp, qn, w);
       double dn[2 * NH], un[2 * NH], wn[2 * NH];
@@ -391,7 +404,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
       j0 = j1, j1 = u;
     }
   }
-  loadq(base + ghost_index(s0 + 1, n, lo, hi) * stride);
+  load_cell(s0 + 1);
   // In the loop the cell to prefetch, s0+2+p, is never below 0, so its ghost map (O1) is: itself below n, else
   // (periodic) itself minus n, reduced once or twice more when n < 3, or (extrapolation) n-1.  Offsets advance
   // by one stride per step.
@@ -416,7 +429,11 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
       gl -= gl >= nwrap ? nwrap : 0;
       gl -= gl >= nwrap ? nwrap : 0;
       gl = min(gl, n - 1);
-      if (BF || p <= L) loadq(base + gl * stride);
+      if (HALO_DIR && hi == BC_HALO && cl >= n) {
+        if (BF || p <= L) loadh(kp.halo_hi, min(cl - n, 2));
+      } else {
+        if (BF || p <= L) loadq(base + gl * stride);
+      }
     }
     ++cl;
     if ((ACCUM || STAGE >= 1) && (BF || p >= 2)) {  // operands of this step's update (BF, p < 2: a valid cell, unused)
@@ -907,6 +924,23 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
   }()
 #endif
 
+template <int N, int D, int WV>
+static cudaError_t launch_rk3_stage(mfc_grid* g, double* q, double dt, int stage) {
+  if constexpr (WV >= 3 && N != 2) return cudaErrorInvalidValue;
+  else {
+    if (stage == 1) return launch_stage<N, D, WV, 1>(g, q, g->Lq, q, dt);
+    if (stage == 2) return launch_stage<N, D, WV, 2>(g, g->Lq, g->q1, q, dt);
+    return launch_stage<N, D, WV, 3>(g, g->q1, g->Lq, q, dt);
+  }
+}
+
+// MFC_BC_HALO: which ends of the last direction take their ghost layers from the halo arrays
+static bool halo_lo_on(const mfc_grid* g) { return g->kp.bc_lo[g->ndim - 1] == BC_HALO; }
+static bool halo_hi_on(const mfc_grid* g) { return g->kp.bc_hi[g->ndim - 1] == BC_HALO; }
+static bool halo_missing(const mfc_grid* g) {
+  return (halo_lo_on(g) && !g->kp.halo_lo) || (halo_hi_on(g) && !g->kp.halo_hi);
+}
+
 static mfc_status use_device(const mfc_grid* g) {
   CK(cudaSetDevice(g->device));
   return MFC_OK;
@@ -927,8 +961,11 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
     if (p->n[d] < 1) return fail(MFC_ERR_ARG, "mfc_init_grid: n[d] must be >= 1");
     if (d >= p->ndim && p->n[d] != 1) return fail(MFC_ERR_ARG, "mfc_init_grid: n[d] must be 1 for d >= ndim");
     if (d < p->ndim && !(p->dx[d] > 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: dx[d] must be > 0");
-    if (p->bc_lo[d] != MFC_BC_PERIODIC && p->bc_lo[d] != MFC_BC_EXTRAP) return fail(MFC_ERR_ARG, "mfc_init_grid: bad bc_lo");
-    if (p->bc_hi[d] != MFC_BC_PERIODIC && p->bc_hi[d] != MFC_BC_EXTRAP) return fail(MFC_ERR_ARG, "mfc_init_grid: bad bc_hi");
+    const bool halo_ok = p->ndim >= 2 && d == p->ndim - 1;  // MFC_BC_HALO: last direction of a 2-D / 3-D grid only
+    if (p->bc_lo[d] != MFC_BC_PERIODIC && p->bc_lo[d] != MFC_BC_EXTRAP && !(halo_ok && p->bc_lo[d] == MFC_BC_HALO))
+      return fail(MFC_ERR_ARG, "mfc_init_grid: bad bc_lo");
+    if (p->bc_hi[d] != MFC_BC_PERIODIC && p->bc_hi[d] != MFC_BC_EXTRAP && !(halo_ok && p->bc_hi[d] == MFC_BC_HALO))
+      return fail(MFC_ERR_ARG, "mfc_init_grid: bad bc_hi");
     if ((p->bc_lo[d] == MFC_BC_PERIODIC) != (p->bc_hi[d] == MFC_BC_PERIODIC))
       return fail(MFC_ERR_ARG, "mfc_init_grid: periodic must be set on both ends of a direction");
     cells *= p->n[d];
@@ -1043,6 +1080,7 @@ mfc_status mfc_prim_from_cons(mfc_grid* g, const double* q, double* w) {
 mfc_status mfc_rhs_dirs(mfc_grid* g, const double* q, double* rhs, int dir_mask) {
   if (!g || !q || !rhs) return fail(MFC_ERR_ARG, "mfc_rhs: NULL argument");
   if (q == rhs) return fail(MFC_ERR_ARG, "mfc_rhs: q and rhs must not alias");
+  if (halo_missing(g)) return fail(MFC_ERR_ARG, "mfc_rhs: MFC_BC_HALO without mfc_set_halo");
   if (mfc_status s = use_device(g)) return s;
   CK(MFC_DISPATCH_W(g, (launch_rhs<N, D, WV>(g, q, rhs, dir_mask))));
   return MFC_OK;
@@ -1054,8 +1092,52 @@ mfc_status mfc_rk3_steps(mfc_grid* g, double* q, double dt, int nsteps) {
   if (!g || !q) return fail(MFC_ERR_ARG, "mfc_rk3_step: NULL argument");
   if (nsteps < 0) return fail(MFC_ERR_ARG, "mfc_rk3_steps: nsteps < 0");
   if (!(dt == dt)) return fail(MFC_ERR_ARG, "mfc_rk3_step: dt is NaN");
+  if (halo_lo_on(g) || halo_hi_on(g))
+    return fail(MFC_ERR_ARG, "mfc_rk3_step: with MFC_BC_HALO the halos must be refreshed before every stage: use mfc_rk3_stage");
   if (mfc_status s = use_device(g)) return s;
   for (int s = 0; s < nsteps; ++s) CK(MFC_DISPATCH_W(g, (launch_rk3<N, D, WV>(g, q, dt))));
+  return MFC_OK;
+}
+
+mfc_status mfc_rk3_stage(mfc_grid* g, double* q, double dt, int stage) {
+  if (!g || !q) return fail(MFC_ERR_ARG, "mfc_rk3_stage: NULL argument");
+  if (stage < 1 || stage > 3) return fail(MFC_ERR_ARG, "mfc_rk3_stage: stage must be 1, 2 or 3");
+  if (!(dt == dt)) return fail(MFC_ERR_ARG, "mfc_rk3_stage: dt is NaN");
+  if (halo_missing(g)) return fail(MFC_ERR_ARG, "mfc_rk3_stage: MFC_BC_HALO without mfc_set_halo");
+  if (mfc_status s = use_device(g)) return s;
+  CK(MFC_DISPATCH_W(g, (launch_rk3_stage<N, D, WV>(g, q, dt, stage))));
+  return MFC_OK;
+}
+
+mfc_status mfc_stage_input(mfc_grid* g, const double* q, int stage, const double** state_out) {
+  if (!g || !q || !state_out) return fail(MFC_ERR_ARG, "mfc_stage_input: NULL argument");
+  if (stage < 1 || stage > 3) return fail(MFC_ERR_ARG, "mfc_stage_input: stage must be 1, 2 or 3");
+  *state_out = stage == 1 ? q : stage == 2 ? g->Lq : g->q1;
+  return MFC_OK;
+}
+
+mfc_status mfc_pack_halo(mfc_grid* g, const double* q, int stage, double* send_lo, double* send_hi) {
+  if (!g || !q || (!send_lo && !send_hi)) return fail(MFC_ERR_ARG, "mfc_pack_halo: NULL argument");
+  if (stage < 1 || stage > 3) return fail(MFC_ERR_ARG, "mfc_pack_halo: stage must be 1, 2 or 3");
+  const int nl = g->kp.n[g->ndim - 1];
+  if (g->ndim < 2 || nl < 3) return fail(MFC_ERR_ARG, "mfc_pack_halo: needs a 2-D or 3-D grid with at least 3 cells in the last direction");
+  if (mfc_status s = use_device(g)) return s;
+  const double* st = stage == 1 ? q : stage == 2 ? g->Lq : g->q1;
+  const size_t plane = (size_t)(g->kp.ncells / nl);
+  const size_t row = 3 * plane * sizeof(double), pitch = (size_t)g->kp.ncells * sizeof(double);
+  // per variable the three layers next to an end are contiguous: one strided copy per end
+  if (send_lo) CK(cudaMemcpy2DAsync(send_lo, row, st, pitch, row, g->neq, cudaMemcpyDeviceToDevice, g->stream));
+  if (send_hi)
+    CK(cudaMemcpy2DAsync(send_hi, row, st + (size_t)(nl - 3) * plane, pitch, row, g->neq, cudaMemcpyDeviceToDevice, g->stream));
+  return MFC_OK;
+}
+
+mfc_status mfc_set_halo(mfc_grid* g, const double* halo_lo, const double* halo_hi) {
+  if (!g) return fail(MFC_ERR_ARG, "mfc_set_halo: NULL handle");
+  if ((halo_lo_on(g) && !halo_lo) || (halo_hi_on(g) && !halo_hi))
+    return fail(MFC_ERR_ARG, "mfc_set_halo: NULL array for an end with MFC_BC_HALO");
+  g->kp.halo_lo = halo_lo;
+  g->kp.halo_hi = halo_hi;
   return MFC_OK;
 }
 
@@ -1108,6 +1190,7 @@ static mfc_status ensure_staging(mfc_grid* g, bool need_r) {
 
 mfc_status mfc_rhs_host(mfc_grid* g, const double* q_host, double* rhs_host) {
   if (!g || !q_host || !rhs_host) return fail(MFC_ERR_ARG, "mfc_rhs_host: NULL argument");
+  if (halo_missing(g)) return fail(MFC_ERR_ARG, "mfc_rhs_host: MFC_BC_HALO without mfc_set_halo");
   if (mfc_status s = use_device(g)) return s;
   if (mfc_status s = ensure_staging(g, true)) return s;
   CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));
@@ -1120,6 +1203,7 @@ mfc_status mfc_rhs_host(mfc_grid* g, const double* q_host, double* rhs_host) {
 mfc_status mfc_rk3_steps_host(mfc_grid* g, double* q_host, double dt, int nsteps) {
   if (!g || !q_host) return fail(MFC_ERR_ARG, "mfc_rk3_steps_host: NULL argument");
   if (nsteps < 0) return fail(MFC_ERR_ARG, "mfc_rk3_steps_host: nsteps < 0");
+  if (halo_lo_on(g) || halo_hi_on(g)) return fail(MFC_ERR_ARG, "mfc_rk3_steps_host: not available with MFC_BC_HALO");
   if (mfc_status s = use_device(g)) return s;
   if (mfc_status s = ensure_staging(g, false)) return s;
   CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));
@@ -1144,6 +1228,7 @@ static mfc_status advance_impl(mfc_grid* g, double* q, double cfl, int nsteps, d
 mfc_status mfc_advance(mfc_grid* g, double* q, double cfl, int nsteps, double* t_elapsed_host) {
   if (!g || !q) return fail(MFC_ERR_ARG, "mfc_advance: NULL argument");
   if (nsteps < 0 || !(cfl > 0.0)) return fail(MFC_ERR_ARG, "mfc_advance: nsteps < 0 or cfl <= 0");
+  if (halo_lo_on(g) || halo_hi_on(g)) return fail(MFC_ERR_ARG, "mfc_advance: not available with MFC_BC_HALO (use mfc_rk3_stage)");
   if (mfc_status s = use_device(g)) return s;
   return advance_impl(g, q, cfl, nsteps, t_elapsed_host);
 }
@@ -1151,6 +1236,7 @@ mfc_status mfc_advance(mfc_grid* g, double* q, double cfl, int nsteps, double* t
 mfc_status mfc_advance_host(mfc_grid* g, double* q_host, double cfl, int nsteps, double* t_elapsed_host) {
   if (!g || !q_host) return fail(MFC_ERR_ARG, "mfc_advance_host: NULL argument");
   if (nsteps < 0 || !(cfl > 0.0)) return fail(MFC_ERR_ARG, "mfc_advance_host: nsteps < 0 or cfl <= 0");
+  if (halo_lo_on(g) || halo_hi_on(g)) return fail(MFC_ERR_ARG, "mfc_advance_host: not available with MFC_BC_HALO");
   if (mfc_status s = use_device(g)) return s;
   if (mfc_status s = ensure_staging(g, false)) return s;
   CK(cudaMemcpyAsync(g->hq, q_host, state_bytes(g), cudaMemcpyHostToDevice, g->stream));

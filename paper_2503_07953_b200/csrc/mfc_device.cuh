@@ -6,7 +6,7 @@
 
 namespace mfc {
 
-enum { BC_PERIODIC = 0, BC_EXTRAP = 1 };
+enum { BC_PERIODIC = 0, BC_EXTRAP = 1, BC_HALO = 2 };
 enum { WENO_JS = 0, WENO_M = 1, WENO_Z = 2 };  // nonlinear weights (mfc_weno of include/mfc_b200.h)
 
 // Kernel parameters (passed by value; lives in the constant bank of each launch).
@@ -24,6 +24,9 @@ struct KP {
   double gam[2]; // gamma_i and gamma_i pi_inf_i of the two fluids: rho_i c_i^2 = gamma_i p + gamma_i pi_inf_i (eq. 6)
   double gpi[2];
   int* flag;     // sticky non-physical flag (A19)
+  // BC_HALO on the last direction (slab decomposition): the three ghost layers beyond each end, [neq][3][plane]
+  const double* halo_lo;
+  const double* halo_hi;
 };
 
 // O1: logical cell g in [-3, n+2] -> interior cell that supplies its value.

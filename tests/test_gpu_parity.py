@@ -559,3 +559,90 @@ def test_kapila_needs_two_fluids(torch, mfc):
     with pytest.raises(mfc.MfcError) as e:
         mfc.Grid.from_case(replace(make_case(1, 3, (16, 1, 1), W.BC_EXTRAP), model="kapila"))
     assert e.value.status == mfc.MFC_ERR_ARG
+
+
+# ------------------------------------------------------------------ slab decomposition (MFC_BC_HALO), several slabs on one GPU
+def _slabs_on_one_gpu(torch, case, q, k):
+    """k slabs of the global case, all on this GPU, run one after the other (no rank waits on another); the exchange is
+    done here by copying each slab's packed layers into its neighbours' halo arrays"""
+    from paper_2503_07953_b200 import slab as S
+    slabs = [S.Slab(case, rank=r, world=k) for r in range(k)]
+    d = case.ndim - 1
+    qs = []
+    for s in slabs:
+        idx = [slice(None)] * 4
+        idx[3 - d] = slice(s.start, s.start + s.count)
+        qs.append(torch.from_numpy(np.ascontiguousarray(q[tuple(idx)])).cuda())
+
+    def refresh(stage):
+        for s, ql in zip(slabs, qs):
+            s.pack(ql, stage)
+        for s in slabs:
+            if s.below is not None:
+                s.halo_lo.copy_(slabs[s.below].send_hi)
+            if s.above is not None:
+                s.halo_hi.copy_(slabs[s.above].send_lo)
+    return slabs, qs, refresh
+
+
+def _gather(case, slabs, parts):
+    d = case.ndim - 1
+    return np.concatenate([p.cpu().numpy() for p in parts], axis=3 - d)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("k", [1, 2, 3])
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_EXTRAP])
+@pytest.mark.parametrize("ndim,nfluids,n", [(3, 2, (33, 18, 23)), (2, 2, (67, 35, 1)), (3, 3, (20, 9, 13))])
+def test_slabs_reproduce_the_single_domain_bit_for_bit(torch, mfc, ndim, nfluids, n, bc, k):
+    # the halo path only changes where ghost values are read from: the rhs and three RK3 steps of k slabs equal the
+    # single-domain result exactly (k = 1 periodic: the slab is its own neighbour)
+    case = make_case(ndim, nfluids, n, bc)
+    q = rough_state(case, 7)
+    whole = gpu_rhs(torch, mfc, case, q)
+    slabs, qs, refresh = _slabs_on_one_gpu(torch, case, q, k)
+    outs = [torch.full_like(ql, float("nan")) for ql in qs]
+    refresh(1)
+    for s, ql, o in zip(slabs, qs, outs):
+        s.grid.rhs(ql, o)
+        s.grid.check()
+    assert np.array_equal(_gather(case, slabs, outs), whole)
+    # RK3 with the dt of the single domain
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    for _ in range(3):
+        dt = g.cfl_dt(qd, 0.4)
+        dts = [s.grid.cfl_dt(ql, 0.4) for s, ql in zip(slabs, qs)]
+        assert min(dts) == dt                                   # the global dt is the minimum of the local ones
+        g.rk3_step(qd, dt)
+        for stage in (1, 2, 3):
+            refresh(stage)
+            for s, ql in zip(slabs, qs):
+                s.grid.rk3_stage(ql, dt, stage)
+    assert np.array_equal(_gather(case, slabs, qs), qd.cpu().numpy())
+    for s in slabs:
+        s.close()
+    g.close()
+
+
+@pytest.mark.gpu
+def test_single_slab_self_exchange_and_refusals(torch, mfc):
+    from paper_2503_07953_b200 import slab as S
+    case = make_case(3, 2, (24, 12, 16), W.BC_PERIODIC)
+    q = rough_state(case, 2)
+    s = S.Slab(case)                       # world 1, periodic: both neighbours are the slab itself
+    qd = torch.from_numpy(q).cuda()
+    g = mfc.Grid.from_case(case)
+    q2 = qd.clone()
+    for _ in range(2):
+        dt = s.cfl_dt(qd, 0.5)
+        assert dt == g.cfl_dt(q2, 0.5)
+        s.rk3_step(qd, dt)
+        g.rk3_step(q2, dt)
+    assert torch.equal(qd, q2) and s.exchanges == 6
+    with pytest.raises(mfc.MfcError):
+        s.grid.rk3_step(qd, 1e-9)          # a handle with halos cannot run the three stages unattended
+    with pytest.raises(mfc.MfcError):
+        mfc.Grid.from_case(replace(make_case(1, 1, (16, 1, 1), W.BC_EXTRAP), bc_lo=(mfc.BC_HALO, 1, 1)))   # 1-D: refused
+    s.close()
+    g.close()

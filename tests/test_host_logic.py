@@ -142,3 +142,83 @@ def test_replica_launch_path_world_size_2_gloo(tmp_path):
     for r in recs:
         assert r["ms"] == 15.0
         assert r["val"] == pytest.approx(15.0 * 1e6 / (3 * 4 * 1000 * 8 * 2))
+
+
+# ------------------------------------------------------------------ slab decomposition: host logic and the exchange over gloo
+def test_slab_partition_neighbours_and_local_case():
+    from paper_2503_07953_b200 import slab as S
+    import paper_2503_07953_b200 as M
+    assert S.partition(10, 3) == [(0, 4), (4, 3), (7, 3)]
+    assert sum(c for _, c in S.partition(257, 8)) == 257
+    with pytest.raises(ValueError):
+        S.partition(8, 3)                                   # a slab of 2 cells cannot fill a 3-deep halo
+    assert S.neighbours(0, 4, True) == (3, 1) and S.neighbours(3, 4, True) == (2, 0)
+    assert S.neighbours(0, 4, False) == (None, 1) and S.neighbours(3, 4, False) == (2, None)
+    assert S.neighbours(0, 1, True) == (0, 0) and S.neighbours(0, 1, False) == (None, None)
+    case = W.config(5, n=24)                                # extrapolation on every side
+    c0, s0, n0 = S.local_case(case, 0, 3)
+    c2, s2, n2 = S.local_case(case, 2, 3)
+    assert (s0, n0, s2, n2) == (0, 8, 16, 8) and c0.n == (24, 24, 8) and c0.dx == case.dx
+    assert c0.bc_lo[2] == M.BC_EXTRAP and c0.bc_hi[2] == M.BC_HALO and c2.bc_lo[2] == M.BC_HALO and c2.bc_hi[2] == M.BC_EXTRAP
+    assert c0.bc_lo[:2] == case.bc_lo[:2]
+    cp, _, _ = S.local_case(W.config(4, n=24), 1, 2)        # periodic: halos on both ends of every slab
+    assert cp.bc_lo[2] == M.BC_HALO and cp.bc_hi[2] == M.BC_HALO
+    with pytest.raises(ValueError):
+        S.local_case(W.config(1), 0, 2)                     # 1-D
+
+
+_SLAB_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch, torch.distributed as dist
+from paper_2503_07953_b200 import slab as S
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+res = dict(rank=rank)
+for periodic in (True, False):
+    below, above = S.neighbours(rank, world, periodic)
+    mk = lambda v: torch.full((12,), float(v), dtype=torch.float64)
+    send_lo, send_hi = mk(10 * rank + 1), mk(10 * rank + 2)
+    halo_lo = mk(-1) if below is not None else None
+    halo_hi = mk(-1) if above is not None else None
+    S.exchange(send_lo if below is not None else None, send_hi if above is not None else None, halo_lo, halo_hi,
+               rank, below, above, dist, None)
+    res["p" if periodic else "e"] = [None if halo_lo is None else halo_lo.tolist(), None if halo_hi is None else halo_hi.tolist(),
+                                     below, above]
+    t = torch.tensor([1.0 + rank]); dist.all_reduce(t, op=dist.ReduceOp.MIN); res["min"] = float(t)
+print(json.dumps(res))
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_exchange_over_gloo(tmp_path, world):
+    """every slab receives its lower neighbour's top layers as halo_lo and its upper neighbour's bottom layers as halo_hi —
+    also when both neighbours are the same peer (two slabs, periodic), where only the posting order tells the two
+    messages apart"""
+    script = tmp_path / "slab_worker.py"
+    script.write_text(_SLAB_WORKER.format(root=ROOT))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(world),
+                          "--master-addr", "127.0.0.1", "--master-port", str(29580 + world), str(script)],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    recs = {}
+    for l in out.stdout.replace("}{", "}\n{").splitlines():
+        if l.startswith("{"):
+            r = json.loads(l)
+            recs[r["rank"]] = r
+    assert sorted(recs) == list(range(world))
+    for rank, r in recs.items():
+        assert r["min"] == 1.0
+        for key in ("p", "e"):
+            lo, hi, below, above = r[key]
+            if below is None:
+                assert lo is None
+            else:
+                assert lo == [10.0 * below + 2] * 12          # the lower neighbour's send_hi
+            if above is None:
+                assert hi is None
+            else:
+                assert hi == [10.0 * above + 1] * 12          # the upper neighbour's send_lo
+        assert r["p"][2] == (rank - 1) % world and r["p"][3] == (rank + 1) % world
