@@ -198,6 +198,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--weno", default="js", choices=["js", "m", "z"],
                     help="nonlinear weights: js = BASELINE.json's WENO5-JS (default), m = mapped (the paper's default), z = WENO-Z")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default, DESIGN.md §9) or one periodic domain of N stacked slabs "
+                         "exchanging 3-layer halos over NCCL (weak scaling: every rank owns one configuration-sized slab)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -223,7 +226,21 @@ def main():
 
     case = dataclasses.replace(W.config(args.config, n=args.n), weno=args.weno)
     q0 = W.initial_state(case)
-    g = M.Grid.from_case(case, device=local_rank)
+    slab = None
+    if args.decomp == "slab":
+        from paper_2503_07953_b200 import slab as S
+        d = case.ndim - 1
+        if case.ndim < 2 or case.bc_lo[d] != W.BC_PERIODIC:
+            raise SystemExit("bench.py --decomp slab: needs a 2-D/3-D configuration periodic in its last direction (config 4)")
+        n_glob = list(case.n)
+        n_glob[d] *= world                      # the rank's block repeated `world` times along the last direction
+        slab = S.Slab(dataclasses.replace(case, n=tuple(n_glob)), rank, world, local_rank,
+                      torch.distributed if world > 1 else None)
+        g = slab.grid
+        advance = lambda q, cfl, n: slab.advance(q, cfl, n)
+    else:
+        g = M.Grid.from_case(case, device=local_rank)
+        advance = lambda q, cfl, n: g.advance(q, cfl, n)
     qd = torch.from_numpy(q0).cuda()
     cells, neq = case.cells, case.neq
 
@@ -235,7 +252,7 @@ def main():
 
     # ---- device-resident timing: the headline value
     for _ in range(args.warmup):
-        g.advance(qd, case.cfl, 1)
+        advance(qd, case.cfl, 1)
     g.check()
     sampler = ClockSampler(local_rank)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -243,7 +260,7 @@ def main():
     barrier()
     sampler.start()
     ev0.record()
-    g.advance(qd, case.cfl, args.steps)
+    advance(qd, case.cfl, args.steps)
     ev1.record()
     torch.cuda.synchronize()
     clocks = sampler.stop()
@@ -255,7 +272,7 @@ def main():
 
     # ---- per-kernel device times (CUDA events around every launch, on the launching stream) for the roofline
     g.set_profiling(True)
-    g.advance(qd, case.cfl, args.steps)
+    advance(qd, case.cfl, args.steps)
     prof = g.get_profile()
     g.set_profiling(False)
     tot_ms = sum(v[0] for v in prof.values())
@@ -288,18 +305,28 @@ def main():
     e2e = None
     if not args.no_e2e:
         qh = torch.from_numpy(q0.copy()).pin_memory()
+        if slab is None:
+            step_host = lambda: g.advance_host(qh, case.cfl, 1)  # syncs inside
+            call = "mfc_advance_host(q_host pinned, cfl, 1) per step"
+        else:
+            def step_host():  # the slab path has no host-buffer entry point: the copies are made here
+                qd.copy_(qh, non_blocking=True)
+                slab.advance(qd, case.cfl, 1)
+                qh.copy_(qd, non_blocking=True)
+                torch.cuda.synchronize()
+            call = "pinned H2D copy + Slab.advance(q, cfl, 1) + D2H copy per step"
         for _ in range(2):
-            g.advance_host(qh, case.cfl, 1)
+            step_host()
         n_e2e = max(2, min(args.steps, 10))
         barrier()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
-            g.advance_host(qh, case.cfl, 1)  # syncs inside
+            step_host()
         sec = time.perf_counter() - t0
         e_ms = reduce_max_ms(sec * 1e3, world)
         e2e = {"value": grind_ns(e_ms, n_e2e, cells, neq, world), "unit": UNIT, "h2d_bytes_per_step": 8 * neq * cells,
                "d2h_bytes_per_step": 8 * neq * cells, "steps": n_e2e, "ms_per_step": e_ms / n_e2e,
-               "call": "mfc_advance_host(q_host pinned, cfl, 1) per step"}
+               "call": call}
         del qh
 
     out = {
@@ -307,7 +334,8 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": case.name, "grid": list(case.n[:case.ndim]), "cells": cells, "neq": neq, "nfluids": case.nfluids,
-                   "weno": {"js": "WENO5-JS", "m": "WENO5-M (mapped)", "z": "WENO5-Z"}[args.weno], "rhs_evals_per_step": 3, "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "weno": {"js": "WENO5-JS", "m": "WENO5-M (mapped)", "z": "WENO5-Z"}[args.weno], "rhs_evals_per_step": 3, "parallelism": ("slabs along the last direction, %d x 3-layer halo exchanges per step" % (3 * 2) if slab is not None
+                                   else "replicas only" if world > 1 else "single GPU"),
                    "l2": "inputs larger than L2 (state array %.0f MB vs 126 MB L2)" % (8e-6 * neq * cells) if 8 * neq * cells > 3e8
                    else "working set fits L2: latency/L2-bound configuration, roofline target does not apply"},
         "cell_updates_per_s": cells * world * args.steps / (ms * 1e-3),
