@@ -146,9 +146,8 @@ __constant__ double WC[W_COUNT] = {13.0 / 3.0, 0.3, 0.6, 0.1, 5.0 / 60.0, -2.0 /
 
 __device__ __forceinline__ double weno5_u(double t, double eps4) { return fma(WCV(W_C133) * t, t, eps4); }
 
-// One reconstructed value c + sum_r A_r Q_r / sum_r A_r from unnormalised weights A_r that already hold the ideal
-// weights' ratios (A = (A0, A1, A2) for stencils 0, 1, 2) and the candidate deviations Q_r scaled by the same
-// constants — see weno5_core for the JS/Z case.  One reciprocal.
+// Both face values of a cell from its centre value c, the first differences d1..d4 of its stencil and
+// u_k = 13/3 t_k^2 + 4 eps of its three second differences; WV = WENO_JS / WENO_M / WENO_Z selects the nonlinear weights.
 template <int WV>
 __device__ __forceinline__ void weno5_core(double c, double d1, double d2, double d3, double d4, double u0, double u1,
                                            double u2, double& L, double& R) {
