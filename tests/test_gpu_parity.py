@@ -646,3 +646,30 @@ def test_single_slab_self_exchange_and_refusals(torch, mfc):
         mfc.Grid.from_case(replace(make_case(1, 1, (16, 1, 1), W.BC_EXTRAP), bc_lo=(mfc.BC_HALO, 1, 1)))   # 1-D: refused
     s.close()
     g.close()
+
+
+# ------------------------------------------------------------------ mfc_advance (CFL reduction + RK3 step, nsteps times in one call)
+@pytest.mark.gpu
+@pytest.mark.parametrize("index,n,nsteps", [(1, None, 40), (2, None, 25), (3, 96, 12), (4, 40, 8), (5, 32, 6)])
+def test_advance_equals_cfl_dt_plus_rk3_step_bit_for_bit(torch, mfc, index, n, nsteps):
+    # what bench.py times: the same kernels as the caller's own loop of mfc_cfl_dt + mfc_rk3_step, so the same bits
+    case = W.config(index, n=n)
+    q = W.initial_state(case)
+    g = mfc.Grid.from_case(case)
+    qa, qb = torch.from_numpy(q).cuda(), torch.from_numpy(q).cuda()
+    t_ref = 0.0
+    for _ in range(nsteps):
+        dt = g.cfl_dt(qb, case.cfl)
+        g.rk3_step(qb, dt)
+        t_ref += dt
+    t = g.advance(qa, case.cfl, nsteps)
+    g.check()
+    assert t == t_ref and torch.equal(qa, qb)
+    # and against the oracle's own dt for the state reached
+    assert g.cfl_dt(qa, case.cfl) == O.Oracle(case).cfl_dt(qa.cpu().numpy(), case.cfl)
+    # a second call continues from the state the first one left
+    t2 = g.advance(qa, case.cfl, 2)
+    dt1 = g.cfl_dt(qb, case.cfl); g.rk3_step(qb, dt1)
+    dt2 = g.cfl_dt(qb, case.cfl); g.rk3_step(qb, dt2)
+    assert t2 == dt1 + dt2 and torch.equal(qa, qb)
+    g.close()
