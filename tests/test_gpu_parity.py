@@ -673,3 +673,46 @@ def test_advance_equals_cfl_dt_plus_rk3_step_bit_for_bit(torch, mfc, index, n, n
     dt2 = g.cfl_dt(qb, case.cfl); g.rk3_step(qb, dt2)
     assert t2 == dt1 + dt2 and torch.equal(qa, qb)
     g.close()
+
+
+# ------------------------------------------------------------------ out-of-bounds guard (compute-sanitizer is not available on the pool)
+@pytest.mark.gpu
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_EXTRAP])
+@pytest.mark.parametrize("ndim,nfluids,n", [(1, 2, (5, 1, 1)), (1, 1, (1000, 1, 1)), (2, 2, (67, 35, 1)), (2, 3, (3, 2, 1)),
+                                            (3, 2, (33, 18, 11)), (3, 3, (40, 9, 13)), (3, 2, (2, 2, 2)), (3, 2, (70, 3, 5))])
+def test_kernels_stay_inside_their_arrays(torch, mfc, ndim, nfluids, n, bc):
+    # q and rhs sit in the middle of larger allocations filled with a sentinel: no kernel of the path may write outside
+    # [neq*cells) of either, mfc_rhs must leave q untouched, and two RK3 steps must leave rhs's allocation untouched
+    case = make_case(ndim, nfluids, n, bc)
+    q = rough_state(case, 4)
+    cnt = q.size
+    pad = 4096
+    SENT = -7.25e300
+
+    def guarded(fill=None):
+        buf = torch.full((cnt + 2 * pad,), SENT, dtype=torch.float64, device="cuda")
+        mid = buf[pad:pad + cnt]
+        if fill is not None:
+            mid.copy_(torch.from_numpy(fill.reshape(-1)))
+        return buf, mid
+
+    def intact(buf):
+        return bool((buf[:pad] == SENT).all()) and bool((buf[pad + cnt:] == SENT).all())
+
+    qbuf, qd = guarded(q)
+    rbuf, rd = guarded()
+    g = mfc.Grid.from_case(case)
+    g.rhs(qd, rd)
+    g.check()
+    assert intact(qbuf) and intact(rbuf)
+    assert np.array_equal(qd.cpu().numpy().reshape(q.shape), q)            # the swept state is read-only
+    assert bool(torch.isfinite(rd).all()) and not bool((rd == SENT).any())  # every cell of rhs was written
+    before = rbuf.clone()
+    dt = g.cfl_dt(qd, 0.3)
+    g.rk3_step(qd, dt)
+    g.rk3_step(qd, dt)
+    g.prim_from_cons(qd, rd)
+    g.check()
+    assert intact(qbuf) and intact(rbuf) and bool(torch.isfinite(qd).all())
+    assert torch.equal(before[:pad], rbuf[:pad])
+    g.close()
