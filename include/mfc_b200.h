@@ -82,7 +82,8 @@ typedef struct {
   const double *gamma;   /* host, N values: gamma_i   of e_i = (p + gamma_i pi_inf_i)/((gamma_i-1) rho_i) */
   const double *pi_inf;  /* host, N values: pi_inf_i; both copied at init */
   int bc_lo[3], bc_hi[3];/* mfc_bc per direction and end */
-  double weno_eps;       /* epsilon of the WENO weights, PAPER.md:163/566 (A4); > 0 */
+  double weno_eps;       /* epsilon of the WENO weights, PAPER.md:163/566 (A4); >= 1e-75 (the kernels evaluate the weights
+                          * in product form, whose smallest term is (4 eps)^4) */
   double alpha_floor;    /* volume-fraction floor of the RK-stage clamp (A10) */
   int clamp;             /* 0: no clamp; 1: apply A10 after every RK stage */
   int weno;              /* mfc_weno: nonlinear weights of the reconstruction; 0 = MFC_WENO_JS */

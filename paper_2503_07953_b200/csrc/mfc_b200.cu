@@ -974,6 +974,8 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   for (int i = 0; i < p->nfluids; ++i)
     if (!(p->gamma[i] > 1.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: gamma_i must be > 1");
   if (!(p->weno_eps > 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: weno_eps must be > 0");
+  // the weights are evaluated in product form: (4 eps)^4 must not underflow where all three indicators vanish
+  if (p->weno_eps < 1e-75) return fail(MFC_ERR_ARG, "mfc_init_grid: weno_eps must be >= 1e-75 (product form of the weights)");
   if (p->model != MFC_MODEL_ALLAIRE && p->model != MFC_MODEL_KAPILA)
     return fail(MFC_ERR_ARG, "mfc_init_grid: model must be MFC_MODEL_ALLAIRE or MFC_MODEL_KAPILA");
   if (p->model == MFC_MODEL_KAPILA && p->nfluids != 2)

@@ -716,3 +716,27 @@ def test_kernels_stay_inside_their_arrays(torch, mfc, ndim, nfluids, n, bc):
     assert intact(qbuf) and intact(rbuf) and bool(torch.isfinite(qd).all())
     assert torch.equal(before[:pad], rbuf[:pad])
     g.close()
+
+
+# ------------------------------------------------------------------ epsilon of the weights (A4): other magnitudes than the configs' 1e-16
+@pytest.mark.gpu
+@pytest.mark.parametrize("weno", ["js", "m", "z"])
+@pytest.mark.parametrize("eps", [1e-6, 1e-40, 1e-70])
+def test_rhs_with_other_weno_eps(torch, mfc, eps, weno):
+    # the product form of the weights must agree with the oracle's quotient form for large and for tiny epsilon, also
+    # where the data are locally constant (all indicators zero: the smallest products, (4 eps)^4)
+    case = replace(make_case(3, 2, (24, 10, 9), W.BC_PERIODIC, eps=eps), weno=weno)
+    q = rough_state(case, 8)
+    q[:, :, :, :8] = q[:, :1, :1, :1]            # a uniform block: stencils with zero smoothness indicators
+    ref, _ = oracle_rhs_with_noise(case, q)
+    got = gpu_rhs(torch, mfc, case, q)
+    assert np.isfinite(got).all()
+    worst, per = rel_err(got, ref, 2, 3)
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.gpu
+def test_weno_eps_below_the_product_form_range_is_refused(torch, mfc):
+    with pytest.raises(mfc.MfcError) as e:
+        mfc.Grid.from_case(make_case(1, 1, (16, 1, 1), W.BC_EXTRAP, eps=1e-80))
+    assert e.value.status == mfc.MFC_ERR_ARG
