@@ -726,6 +726,9 @@ static void default_segments(mfc_grid* g) {
       const long long nseg = (want_threads + cols - 1) / cols;
       long long l = (n + nseg - 1) / nseg;
       if (l < 8) l = 8;
+      // short segments pay 2 extra reconstructions and a 4-cell prologue each: take 32 cells if that still fills
+      // three quarters of the resident threads (2 blocks of MB per SM), measured on config 3: 8 % faster than 8
+      if (l < 32 && n >= 32 && cols * ((n + 31) / 32) * 4 >= (long long)g->num_sms * 2 * MB * 3) l = 32;
       if (l < n) L = (int)l;
     }
     g->seg[d] = L;
