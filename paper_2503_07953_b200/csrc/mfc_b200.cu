@@ -123,7 +123,7 @@ struct XCursor {
 template <int N, int D, bool ACCUM, int STAGE, int WV>
 __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                    double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt,
-                                                   int chunk, unsigned* next_chunk) {
+                                                   int chunk, unsigned* next_chunk, unsigned* reset_other) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
   __shared__ double ring[XW][NEQ][64];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -172,7 +172,9 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
     }
   };
   // chunks of `chunk` consecutive items are handed out dynamically (one atomic per chunk), so that the warps of the
-  // single wave finish together
+  // single wave finish together.  Two counters alternate between launches: this launch zeroes the one the next launch
+  // on the stream will use (no memset between the sweeps).
+  if (blockIdx.x == 0 && threadIdx.x == 0) *reset_other = 0u;
   for (;;) {
   unsigned ck = 0;
   if (lane == 0) ck = atomicAdd(next_chunk, 1u);
@@ -624,7 +626,8 @@ struct mfc_grid {
   double* hr = nullptr;
   unsigned long long* d_red = nullptr;  // [0] = smax bits
   int* d_flag = nullptr;
-  unsigned* d_xnext = nullptr;          // work counter of sweep_x
+  unsigned* d_xnext = nullptr;          // two work counters of sweep_x, used alternately (each launch zeroes the other)
+  int xparity = 0;
   int xchunk = 0;                       // items per chunk (0 = default)
   unsigned long long* h_red = nullptr;  // pinned: [0] smax bits, [1] flag
   int seg[3];
@@ -791,10 +794,11 @@ static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* q
   if (chunk < 1) chunk = 1;
   if (chunk > 16) chunk = 16;
   if (g->xchunk > 0) chunk = g->xchunk;
-  cudaError_t e = cudaMemsetAsync(g->d_xnext, 0, sizeof(unsigned), g->stream);
-  if (e != cudaSuccess) return e;
+  unsigned* cur = g->d_xnext + (g->xparity & 1);
+  unsigned* other = g->d_xnext + ((g->xparity + 1) & 1);
+  g->xparity ^= 1;
   Scope sc(g, MFC_K_SWEEP_X);
-  kern<<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt, (int)chunk, g->d_xnext);
+  kern<<<(unsigned)nb, XW * 32, 0, g->stream>>>(g->kp, q, rhs, seglen, nseg, qn, dt, (int)chunk, cur, other);
   return cudaGetLastError();
 }
 
@@ -1029,7 +1033,7 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   cudaError_t e;
   if ((e = cudaMalloc(&g->q1, bytes)) != cudaSuccess || (e = cudaMalloc(&g->Lq, bytes)) != cudaSuccess ||
       (e = cudaMalloc(&g->d_red, 16)) != cudaSuccess || (e = cudaMalloc(&g->d_flag, sizeof(int))) != cudaSuccess ||
-      (e = cudaMalloc(&g->d_xnext, sizeof(unsigned))) != cudaSuccess ||
+      (e = cudaMalloc(&g->d_xnext, 2 * sizeof(unsigned))) != cudaSuccess ||
       (e = cudaMallocHost(&g->h_red, 16)) != cudaSuccess) {
     mfc_free_grid(g);
     g_err = std::string("mfc_init_grid: allocation failed: ") + cudaGetErrorString(e);
@@ -1039,6 +1043,7 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   g->kp.flag = g->d_flag;
   CK(cudaMemsetAsync(g->d_flag, 0, sizeof(int), g->stream));
   CK(cudaMemsetAsync(g->d_red, 0, 16, g->stream));
+  CK(cudaMemsetAsync(g->d_xnext, 0, 2 * sizeof(unsigned), g->stream));
   *out = g;
   return MFC_OK;
 }
