@@ -188,6 +188,11 @@ mfc_status mfc_hllc_faces(mfc_grid *g, int dir, const double *wL, const double *
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 long long mfc_launch_count(const mfc_grid *g);
 
+/* Measurement aid for the roofline (no part of the path): sustained vector-FP64 throughput of `device` in TFLOP/s
+ * (2 flop per DFMA) from register-resident DFMA chains on all SMs — with two loop-invariant operands (the pipe's
+ * issue rate) and with three distinct, changing register operands.  Host pointers; syncs. */
+mfc_status mfc_measure_fp64(int device, void *stream, double *dfma_tflops_host, double *dfma3_tflops_host);
+
 /* Tuning knob (benchmarks/tests only): cells per thread segment along the sweep direction, per direction;
  * 0 keeps the library's choice.  Results do not depend on it beyond round-off-free re-partitioning
  * (each face flux is computed from the same inputs wherever the segment boundaries fall). */

@@ -20,7 +20,7 @@ EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "m
            "mfc_rhs_dirs", "mfc_rk3_step", "mfc_rk3_steps", "mfc_cfl_dt", "mfc_check", "mfc_rhs_host",
            "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
            "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error", "mfc_set_halo", "mfc_rk3_stage",
-           "mfc_stage_input", "mfc_pack_halo")
+           "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64")
 
 
 KERNEL_CLASSES = ("prim", "sweep_x", "sweep_y", "sweep_z", "rk", "cfl")
@@ -82,8 +82,16 @@ def lib():
         L.mfc_rk3_stage.argtypes = [vp, dp, C.c_double, C.c_int]
         L.mfc_stage_input.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_void_p)]
         L.mfc_pack_halo.argtypes = [vp, dp, C.c_int, dp, dp]
+        L.mfc_measure_fp64.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
     return _lib
+
+
+def measure_fp64(device=0):
+    """(TFLOP/s of DFMA chains with two loop-invariant operands, with three distinct register operands) on `device`"""
+    a, b = C.c_double(), C.c_double()
+    _ck(lib().mfc_measure_fp64(int(device), None, C.byref(a), C.byref(b)))
+    return a.value, b.value
 
 
 def _ck(status):

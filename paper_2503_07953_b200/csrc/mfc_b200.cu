@@ -609,6 +609,27 @@ __global__ void __launch_bounds__(PB) hllc_unit_kernel(const __grid_constant__ K
   uf[t] = u;
 }
 
+// ------------------------------------------------------------------------------------------------ FP64 peak probe
+// DFMA chains on registers, 8 independent chains per thread, 16 warps per SM (mfc_measure_fp64).
+// MODE 0: x = fma(x, a, b) with loop-invariant a, b — the pipe's issue rate.  MODE 1: x_i = fma(x_i, x_j, x_k) with three
+// distinct, changing register operands — what an FP64 instruction costs when it reads three different registers.
+template <int MODE>
+__global__ void __launch_bounds__(128) dfma_probe_kernel(double* out, int iters, double a, double b) {
+  double x[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) x[i] = 1.0 + 1e-3 * threadIdx.x + i;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int i = 0; i < 8; ++i) x[i] = MODE == 0 ? fma(x[i], a, b) : fma(x[i], x[(i + 1) & 7], x[(i + 3) & 7]);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += x[i];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace mfc
 
 // ================================================================================================ host side
@@ -1278,6 +1299,45 @@ mfc_status mfc_hllc_faces(mfc_grid* g, int dir, const double* wL, const double* 
   if (mfc_status s = use_device(g)) return s;
   if (count == 0) return MFC_OK;
   CK(MFC_DISPATCH(g, (launch_hllc_unit<N, D>(g, dir, wL, wR, count, F, uf))));
+  return MFC_OK;
+}
+
+mfc_status mfc_measure_fp64(int device, void* stream, double* dfma_tflops_host, double* dfma3_tflops_host) {
+  if (!dfma_tflops_host || !dfma3_tflops_host) return fail(MFC_ERR_ARG, "mfc_measure_fp64: NULL argument");
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (device < 0 || device >= ndev) return fail(MFC_ERR_ARG, "mfc_measure_fp64: no such CUDA device");
+  CK(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const int blocks = prop.multiProcessorCount * 4, iters = 40000;  // 4 blocks of 128 threads per SM, ~10 ms per launch
+  double* out = nullptr;
+  CK(cudaMalloc(&out, sizeof(double) * (size_t)blocks * 128));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  double res[2] = {0.0, 0.0};
+  cudaError_t err = cudaSuccess;
+  for (int mode = 0; mode < 2 && err == cudaSuccess; ++mode) {
+    for (int rep = 0; rep < 3; ++rep) {  // first repetition warms up; best of the other two
+      cudaEventRecord(e0, st);
+      if (mode == 0) dfma_probe_kernel<0><<<blocks, 128, 0, st>>>(out, iters, 1.0000001, 1e-9);
+      else dfma_probe_kernel<1><<<blocks, 128, 0, st>>>(out, iters, 1.0000001, 1e-9);
+      cudaEventRecord(e1, st);
+      if ((err = cudaEventSynchronize(e1)) != cudaSuccess) break;
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      const double tf = 2.0 * 32.0 * iters * (double)blocks * 128.0 / (ms * 1e-3) / 1e12;  // 32 DFMA per thread per iteration
+      if (rep > 0 && tf > res[mode]) res[mode] = tf;
+    }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  if (err != cudaSuccess) return cuda_fail(err, "mfc_measure_fp64");
+  *dfma_tflops_host = res[0];
+  *dfma3_tflops_host = res[1];
   return MFC_OK;
 }
 
