@@ -42,6 +42,7 @@ class Case:
     seed: int = DEFAULT_SEED
     builder: str = ""        # which generator below makes q0
     model: str = "allaire"   # volume-fraction equation: "allaire" (no K div u) or "kapila" (eq. 5; two fluids)
+    eta: float = 0.0         # uniform shear viscosity of PAPER.md eq.(1); 0 = inviscid (all five configurations)
     weno: str = "js"         # nonlinear weights: "js" (BASELINE.json), "m" (mapped), "z"
 
     @property

@@ -66,6 +66,7 @@ struct Params {
   int clamp = 0;           // A10
   int recon = RECON_WENO5_JS;
   int model = MODEL_ALLAIRE;
+  T eta = T(0);            // uniform shear viscosity of eq.(1) (A22); 0 = inviscid
 
   int neq() const { return 2 * nfluids + ndim + 1; }  // PAPER.md:704 "two advected species (8 PDEs)" in 3D
   std::size_t cells() const { return std::size_t(n[0]) * n[1] * n[2]; }
@@ -418,7 +419,79 @@ struct Solver {
         }
       }
     }
+    if (P.eta > T(0) && dir_mask == 7) add_viscous(q, rhs_out);
     return bad;
+  }
+
+  // O8 (eqs.(1),(2); reading A22): viscous part of the momentum and energy equations,
+  //   d(rho u_m)/dt += d/dx_d T_md,   dE/dt += d/dx_d (T_md u_m),   T = 2 eta (D - tr(D) I/3),  D = (grad u + grad u^T)/2,
+  // i.e. T_md = eta (du_m/dx_d + du_d/dx_m) - (2/3) eta delta_md div u, with one uniform eta.  The paper prints no
+  // discretisation; the reading is the second-order central one at face centres (the paper's ref. [7]): at the face
+  // between cells i and i+1 along d
+  //   du_m/dx_d = (u_m[i+1] - u_m[i])/dx_d,
+  //   du_m/dx_e = mean over the two cells of (u_m[.,e+1] - u_m[.,e-1])/(2 dx_e)   (e != d),
+  //   u_m(face) = (u_m[i] + u_m[i+1])/2,
+  // and the cell gets (flux at i+1/2 - flux at i-1/2)/dx_d.  Ghost velocities by the index map O1 in every direction.
+  T vel(const T* q, int m, int i, int j, int k) const {
+    int c[3] = {i, j, k};
+    for (int d = 0; d < 3; ++d) c[d] = d < P.ndim ? ghost_index(c[d], P.n[d], P.bc_lo[d], P.bc_hi[d]) : 0;
+    T rho = T(0);
+    for (int f = 0; f < P.nfluids; ++f) rho = rho + q[idx(P.i_arho(f), c[0], c[1], c[2])];
+    return q[idx(P.i_mom(m), c[0], c[1], c[2])] / rho;
+  }
+
+  // viscous flux through the face between cell (i,j,k) and its neighbour one step up in direction d:
+  // Tm[m] = T_md, *G = sum_m T_md u_m(face)
+  void viscous_face(const T* q, int d, int i, int j, int k, T* Tm, T* G) const {
+    const int D = P.ndim;
+    int a[3] = {i, j, k}, b[3] = {i, j, k};
+    b[d] += 1;
+    T grad[3][3];  // grad[m][e] = du_m/dx_e at the face
+    T uf[3];
+    for (int m = 0; m < D; ++m) {
+      const T ua = vel(q, m, a[0], a[1], a[2]), ub = vel(q, m, b[0], b[1], b[2]);
+      uf[m] = (ua + ub) / T(2);
+      for (int e = 0; e < D; ++e) {
+        if (e == d) {
+          grad[m][e] = (ub - ua) / P.dx[d];
+        } else {
+          int ap[3] = {a[0], a[1], a[2]}, am[3] = {a[0], a[1], a[2]}, bp[3] = {b[0], b[1], b[2]}, bm[3] = {b[0], b[1], b[2]};
+          ap[e] += 1; am[e] -= 1; bp[e] += 1; bm[e] -= 1;
+          const T ga = (vel(q, m, ap[0], ap[1], ap[2]) - vel(q, m, am[0], am[1], am[2])) / (T(2) * P.dx[e]);
+          const T gb = (vel(q, m, bp[0], bp[1], bp[2]) - vel(q, m, bm[0], bm[1], bm[2])) / (T(2) * P.dx[e]);
+          grad[m][e] = (ga + gb) / T(2);
+        }
+      }
+    }
+    T div = T(0);
+    for (int m = 0; m < D; ++m) div = div + grad[m][m];
+    *G = T(0);
+    for (int m = 0; m < D; ++m) {
+      Tm[m] = P.eta * (grad[m][d] + grad[d][m]);
+      if (m == d) Tm[m] = Tm[m] - (T(2) * P.eta / T(3)) * div;
+      *G = *G + Tm[m] * uf[m];
+    }
+  }
+
+  void add_viscous(const T* q, T* rhs_out) const {
+    const int D = P.ndim;
+#pragma omp parallel for schedule(static)
+    for (long k = 0; k < P.n[2]; ++k)
+      for (int j = 0; j < P.n[1]; ++j)
+        for (int i = 0; i < P.n[0]; ++i)
+          for (int d = 0; d < D; ++d) {
+            int lo[3] = {i, j, (int)k};
+            lo[d] -= 1;
+            T Tp[3], Tm_[3], Gp, Gm;
+            viscous_face(q, d, i, j, (int)k, Tp, &Gp);
+            viscous_face(q, d, lo[0], lo[1], lo[2], Tm_, &Gm);
+            for (int m = 0; m < D; ++m) {
+              std::size_t t = idx(P.i_mom(m), i, j, (int)k);
+              rhs_out[t] = rhs_out[t] + (Tp[m] - Tm_[m]) / P.dx[d];
+            }
+            std::size_t t = idx(P.i_E(), i, j, (int)k);
+            rhs_out[t] = rhs_out[t] + (Gp - Gm) / P.dx[d];
+          }
   }
 
   void clamp_all(T* q) const {

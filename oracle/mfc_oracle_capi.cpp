@@ -27,6 +27,7 @@ typedef struct {
   int clamp;
   int recon;
   int model;
+  double eta;
 } oracle_params;
 
 }  // extern "C"
@@ -53,6 +54,7 @@ Params<T> convert(const oracle_params* p) {
   P.clamp = p->clamp;
   P.recon = p->recon;
   P.model = p->model;
+  P.eta = T(p->eta);
   P.derive();
   return P;
 }

@@ -23,7 +23,7 @@ class OracleParams(C.Structure):
     _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("dx", C.c_double * 3), ("nfluids", C.c_int),
                 ("gamma", C.c_double * _MAXF), ("pi_inf", C.c_double * _MAXF),
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
-                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("recon", C.c_int), ("model", C.c_int)]
+                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("recon", C.c_int), ("model", C.c_int), ("eta", C.c_double)]
 
 
 _lib = None
@@ -84,6 +84,7 @@ def make_params(case, recon=None):
     p.clamp = int(case.clamp)
     p.recon = recon
     p.model = MODEL_BY_NAME[getattr(case, "model", "allaire")]
+    p.eta = float(getattr(case, "eta", 0.0))
     return p
 
 
