@@ -143,7 +143,7 @@ def run_reference(args, rank):
     import mfc_workloads as W
     from oracle import oracle as O
     n_ref = {1: None, 2: None, 3: 256, 4: 64, 5: 56}[args.config]
-    case = dataclasses.replace(W.config(args.config, n=n_ref), weno=args.weno)
+    case = dataclasses.replace(W.config(args.config, n=n_ref), weno=args.weno, model=args.model, eta=args.eta)
     q = W.initial_state(case)
     orc = O.Oracle(case)
     dt = orc.cfl_dt(q, case.cfl)
@@ -167,11 +167,11 @@ def run_reference(args, rank):
     }))
 
 
-def cpu_baseline(config_index, weno="js", budget_s=20.0):
+def cpu_baseline(config_index, weno="js", model="allaire", eta=0.0, budget_s=20.0):
     import mfc_workloads as W
     from oracle import oracle as O
     n_ref = {1: None, 2: None, 3: 512, 4: 128, 5: 96}[config_index]
-    case = dataclasses.replace(W.config(config_index, n=n_ref), weno=weno)
+    case = dataclasses.replace(W.config(config_index, n=n_ref), weno=weno, model=model, eta=eta)
     q = W.initial_state(case)
     orc = O.Oracle(case)
     dt = orc.cfl_dt(q, case.cfl)
@@ -198,6 +198,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--weno", default="js", choices=["js", "m", "z"],
                     help="nonlinear weights: js = BASELINE.json's WENO5-JS (default), m = mapped (the paper's default), z = WENO-Z")
+    ap.add_argument("--model", default="allaire", choices=["allaire", "kapila"], help="volume-fraction equation (kapila: two fluids)")
+    ap.add_argument("--eta", type=float, default=0.0, help="uniform shear viscosity (0: inviscid, BASELINE.json)")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default, DESIGN.md §9) or one periodic domain of N stacked slabs "
                          "exchanging 3-layer halos over NCCL (weak scaling: every rank owns one configuration-sized slab)")
@@ -224,7 +226,7 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    case = dataclasses.replace(W.config(args.config, n=args.n), weno=args.weno)
+    case = dataclasses.replace(W.config(args.config, n=args.n), weno=args.weno, model=args.model, eta=args.eta)
     q0 = W.initial_state(case)
     slab = None
     if args.decomp == "slab":
@@ -340,7 +342,7 @@ def main():
         "ms_per_step": ms / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": case.name, "grid": list(case.n[:case.ndim]), "cells": cells, "neq": neq, "nfluids": case.nfluids,
-                   "weno": {"js": "WENO5-JS", "m": "WENO5-M (mapped)", "z": "WENO5-Z"}[args.weno], "rhs_evals_per_step": 3, "parallelism": ("slabs along the last direction, %d x 3-layer halo exchanges per step" % (3 * 2) if slab is not None
+                   "weno": {"js": "WENO5-JS", "m": "WENO5-M (mapped)", "z": "WENO5-Z"}[args.weno], "model": args.model, "eta": args.eta, "rhs_evals_per_step": 3, "parallelism": ("slabs along the last direction, %d x 3-layer halo exchanges per step" % (3 * 2) if slab is not None
                                    else "replicas only" if world > 1 else "single GPU"),
                    "l2": "inputs larger than L2 (state array %.0f MB vs 126 MB L2)" % (8e-6 * neq * cells) if 8 * neq * cells > 3e8
                    else "working set fits L2: latency/L2-bound configuration, roofline target does not apply"},
@@ -349,7 +351,7 @@ def main():
         "paper_context": "PAPER.md:720-726 Table 1 (other hardware, whole step): GH200 0.32, H100 SXM 0.38, A100 0.62 ns",
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.config, args.weno)
+        out["cpu_baseline"] = cpu_baseline(args.config, args.weno, args.model, args.eta)
     if rank == 0:
         print(json.dumps(out))
     g.close()

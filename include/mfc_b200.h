@@ -88,6 +88,9 @@ typedef struct {
   int clamp;             /* 0: no clamp; 1: apply A10 after every RK stage */
   int weno;              /* mfc_weno: nonlinear weights of the reconstruction; 0 = MFC_WENO_JS */
   int model;             /* mfc_model: 0 = MFC_MODEL_ALLAIRE; MFC_MODEL_KAPILA needs nfluids == 2 */
+  double eta;            /* uniform shear viscosity of the viscous stress T = 2 eta (D - tr(D) I/3), PAPER.md:63-67 (eqs. 1-2),
+                          * in the momentum and energy equations; second-order central differences at the faces (A22).
+                          * 0 = inviscid (BASELINE.json).  Not available with MFC_BC_HALO. */
   int device;            /* CUDA device ordinal */
   void *stream;          /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
 } mfc_params;

@@ -30,7 +30,7 @@ class MfcParams(C.Structure):
     _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("dx", C.c_double * 3), ("nfluids", C.c_int),
                 ("gamma", C.POINTER(C.c_double)), ("pi_inf", C.POINTER(C.c_double)),
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
-                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("weno", C.c_int), ("model", C.c_int),
+                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("weno", C.c_int), ("model", C.c_int), ("eta", C.c_double),
                 ("device", C.c_int), ("stream", C.c_void_p)]
 
 
@@ -130,7 +130,7 @@ class Grid:
     """Handle of one grid (mfc_init_grid ... mfc_free_grid); methods carry the C names without the prefix."""
 
     def __init__(self, ndim, n, dx, gamma, pi_inf, bc_lo, bc_hi, weno_eps=1e-16, alpha_floor=1e-6, clamp=True,
-                 device=0, stream=None, weno="js", model="allaire"):
+                 device=0, stream=None, weno="js", model="allaire", eta=0.0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2503_07953_b200 needs a CUDA device (there is no CPU fallback)")
@@ -151,6 +151,7 @@ class Grid:
         p.weno_eps, p.alpha_floor, p.clamp = weno_eps, alpha_floor, int(bool(clamp))
         p.weno = WENO_BY_NAME[weno] if isinstance(weno, str) else int(weno)
         p.model = MODEL_BY_NAME[model] if isinstance(model, str) else int(model)
+        p.eta = float(eta)
         p.device = device
         if stream is None:
             stream = torch.cuda.current_stream(device).cuda_stream
@@ -166,7 +167,7 @@ class Grid:
     def from_case(cls, case, device=0, stream=None):
         """case: an mfc_workloads.Case-like object (ndim, n, dx, gamma, pi_inf, bc_lo, bc_hi, weno_eps, alpha_floor, clamp)."""
         return cls(case.ndim, case.n, case.dx, case.gamma, case.pi_inf, case.bc_lo, case.bc_hi, case.weno_eps,
-                   case.alpha_floor, case.clamp, device, stream, getattr(case, "weno", "js"), getattr(case, "model", "allaire"))
+                   case.alpha_floor, case.clamp, device, stream, getattr(case, "weno", "js"), getattr(case, "model", "allaire"), getattr(case, "eta", 0.0))
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -609,6 +609,94 @@ __global__ void __launch_bounds__(PB) hllc_unit_kernel(const __grid_constant__ K
   uf[t] = u;
 }
 
+// ------------------------------------------------------------------------------------------------ viscous terms
+// O8 (eqs.(1),(2); reading A22): T = 2 eta (D - tr(D) I/3) with one uniform eta, second-order
+// central differences at face centres.  Two pointwise kernels, bound by HBM/L2, run BEFORE the sweeps of an RHS evaluation:
+// velocity_kernel writes u_d = (rho u_d)/rho, viscous_kernel overwrites rhs with the viscous rates of momentum and
+// energy (zero for the other equations); the x sweep then accumulates onto it.
+template <int N, int D>
+__global__ void __launch_bounds__(PB) velocity_kernel(const __grid_constant__ KP kp, const double* __restrict__ q,
+                                                      double* __restrict__ vel) {
+  const long long c = (long long)blockIdx.x * PB + threadIdx.x;
+  if (c >= kp.ncells) return;
+  double rho = q[c];
+#pragma unroll
+  for (int i = 1; i < N; ++i) rho = __dadd_rn(rho, q[i * kp.ncells + c]);
+#pragma unroll
+  for (int d = 0; d < D; ++d) vel[d * kp.ncells + c] = __ddiv_rn(q[(N + d) * kp.ncells + c], rho);
+}
+
+template <int N, int D>
+__global__ void __launch_bounds__(PB) viscous_kernel(const __grid_constant__ KP kp, const double* __restrict__ vel,
+                                                     double* __restrict__ rhs) {
+  constexpr int NEQ = 2 * N + D + 1;
+  const long long c = (long long)blockIdx.x * PB + threadIdx.x;
+  if (c >= kp.ncells) return;
+  const int nx = kp.n[0], ny = kp.n[1];
+  int ijk[3];
+  ijk[0] = (int)(c % nx);
+  ijk[1] = (int)((c / nx) % ny);
+  ijk[2] = (int)(c / ((long long)nx * ny));
+  // mapped neighbour indices per direction (O1): nb[d][o+1], o = -1, 0, +1
+  int nb[3][3];
+#pragma unroll
+  for (int d = 0; d < 3; ++d)
+#pragma unroll
+    for (int o = -1; o <= 1; ++o) nb[d][o + 1] = d < D ? ghost_index(ijk[d] + o, kp.n[d], kp.bc_lo[d], kp.bc_hi[d]) : 0;
+  auto U = [&](int m, const int* o) {  // velocity component m at offset o[3] from the cell
+    const long long t = ((long long)nb[2][o[2] + 1] * ny + nb[1][o[1] + 1]) * nx + nb[0][o[0] + 1];
+    return __ldg(vel + m * kp.ncells + t);
+  };
+  double acc[D + 1];
+#pragma unroll
+  for (int m = 0; m <= D; ++m) acc[m] = 0.0;
+#pragma unroll
+  for (int d = 0; d < D; ++d) {
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {  // side 1: face between the cell and its upper neighbour; 0: lower neighbour and the cell
+      int a[3] = {0, 0, 0}, b[3] = {0, 0, 0};
+      a[d] = side - 1;
+      b[d] = side;
+      double grad[D][D], uf[D];
+#pragma unroll
+      for (int m = 0; m < D; ++m) {
+        const double ua = U(m, a), ub = U(m, b);
+        uf[m] = 0.5 * (ua + ub);
+#pragma unroll
+        for (int e = 0; e < D; ++e) {
+          if (e == d) {
+            grad[m][e] = (ub - ua) * kp.inv_dx[d];
+          } else {
+            int ap[3] = {a[0], a[1], a[2]}, am[3] = {a[0], a[1], a[2]}, bp[3] = {b[0], b[1], b[2]}, bm[3] = {b[0], b[1], b[2]};
+            ap[e] += 1, am[e] -= 1, bp[e] += 1, bm[e] -= 1;
+            grad[m][e] = 0.25 * kp.inv_dx[e] * ((U(m, ap) - U(m, am)) + (U(m, bp) - U(m, bm)));
+          }
+        }
+      }
+      double div = 0.0;
+#pragma unroll
+      for (int m = 0; m < D; ++m) div += grad[m][m];
+      const double sgn = side ? kp.inv_dx[d] : -kp.inv_dx[d];
+      double G = 0.0;
+#pragma unroll
+      for (int m = 0; m < D; ++m) {
+        double T = kp.eta * (grad[m][d] + grad[d][m]);
+        if (m == d) T = fma(-(2.0 / 3.0) * kp.eta, div, T);
+        G = fma(T, uf[m], G);
+        acc[m] = fma(sgn, T, acc[m]);
+      }
+      acc[D] = fma(sgn, G, acc[D]);
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < NEQ; ++v) {
+    double r = 0.0;
+    if (v >= N && v < N + D) r = acc[v - N];
+    if (v == N + D) r = acc[D];
+    rhs[v * kp.ncells + c] = r;
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ FP64 peak probe
 // DFMA chains on registers, 8 independent chains per thread, 16 warps per SM (mfc_measure_fp64).
 // MODE 0: x = fma(x, a, b) with loop-invariant a, b — the pipe's issue rate.  MODE 1: x_i = fma(x_i, x_j, x_k) with three
@@ -643,6 +731,7 @@ struct mfc_grid {
   cudaStream_t stream;
   double* q1 = nullptr;     // stage state
   double* Lq = nullptr;     // rhs scratch
+  double* vel = nullptr;    // velocities u_d (D arrays), only when eta > 0
   double* hq = nullptr;     // device staging for the *_host calls (lazy)
   double* hr = nullptr;
   unsigned long long* d_red = nullptr;  // [0] = smax bits
@@ -823,6 +912,21 @@ static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* q
   return cudaGetLastError();
 }
 
+// viscous rates of momentum and energy written over rhs (zero elsewhere); the x sweep accumulates onto them
+template <int N, int D>
+static cudaError_t launch_viscous(mfc_grid* g, const double* q, double* rhs) {
+  const unsigned nb = (unsigned)((g->kp.ncells + PB - 1) / PB);
+  {
+    Scope sc(g, MFC_K_PRIM);
+    velocity_kernel<N, D><<<nb, PB, 0, g->stream>>>(g->kp, q, g->vel);
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  Scope sc(g, MFC_K_PRIM);
+  viscous_kernel<N, D><<<nb, PB, 0, g->stream>>>(g->kp, g->vel, rhs);
+  return cudaGetLastError();
+}
+
 // rhs = L(q) restricted to the directions in mask.  mask == all: x overwrites, y and z accumulate.
 template <int N, int D, int WV>
 static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mask) {
@@ -830,7 +934,10 @@ static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mas
   else {
   const int all = (1 << D) - 1;
   cudaError_t e;
-  if ((mask & all) == all) {
+  if ((mask & all) == all && g->kp.eta > 0.0) {
+    if ((e = launch_viscous<N, D>(g, q, rhs)) != cudaSuccess) return e;
+    if ((e = launch_x<N, D, WV, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
+  } else if ((mask & all) == all) {
     if ((e = launch_x<N, D, WV, false, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   } else {
     if ((e = cudaMemsetAsync(rhs, 0, state_bytes(g), g->stream)) != cudaSuccess) return e;
@@ -851,10 +958,14 @@ static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mas
 template <int N, int D, int WV, int STAGE>
 static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, double* qn, double dt) {
   cudaError_t e;
+  const bool visc = g->kp.eta > 0.0;
+  if (visc)
+    if ((e = launch_viscous<N, D>(g, qs, work)) != cudaSuccess) return e;
   if constexpr (D == 1) {
-    return launch_x<N, D, WV, false, STAGE>(g, qs, work, qn, dt);
+    return visc ? launch_x<N, D, WV, true, STAGE>(g, qs, work, qn, dt) : launch_x<N, D, WV, false, STAGE>(g, qs, work, qn, dt);
   } else {
-    if ((e = launch_x<N, D, WV, false, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
+    e = visc ? launch_x<N, D, WV, true, 0>(g, qs, work, nullptr, 0.0) : launch_x<N, D, WV, false, 0>(g, qs, work, nullptr, 0.0);
+    if (e != cudaSuccess) return e;
     if constexpr (D == 2) {
       return launch_march<N, D, WV, 1, true, STAGE>(g, qs, work, qn, dt);
     } else {
@@ -1008,6 +1119,11 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
     return fail(MFC_ERR_ARG, "mfc_init_grid: model must be MFC_MODEL_ALLAIRE or MFC_MODEL_KAPILA");
   if (p->model == MFC_MODEL_KAPILA && p->nfluids != 2)
     return fail(MFC_ERR_ARG, "mfc_init_grid: MFC_MODEL_KAPILA is defined for two fluids (PAPER.md:78, eq. 5)");
+  if (!(p->eta >= 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: eta must be >= 0");
+  if (p->eta > 0.0)
+    for (int d = 0; d < p->ndim; ++d)
+      if (p->bc_lo[d] == MFC_BC_HALO || p->bc_hi[d] == MFC_BC_HALO)
+        return fail(MFC_ERR_ARG, "mfc_init_grid: viscous terms are not available with MFC_BC_HALO");
   if (p->weno != MFC_WENO_JS && p->weno != MFC_WENO_M && p->weno != MFC_WENO_Z)
     return fail(MFC_ERR_ARG, "mfc_init_grid: weno must be MFC_WENO_JS, MFC_WENO_M or MFC_WENO_Z");
   int ndev = 0;
@@ -1041,6 +1157,7 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   g->kp.alpha_floor = p->alpha_floor;
   g->kp.clamp = p->clamp ? 1 : 0;
   g->kp.kapila = p->model == MFC_MODEL_KAPILA ? 1 : 0;
+  g->kp.eta = p->eta;
   for (int i = 0; i < 2 && i < p->nfluids; ++i) {
     g->kp.gam[i] = p->gamma[i];
     g->kp.gpi[i] = p->gamma[i] * p->pi_inf[i];
@@ -1061,6 +1178,11 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
     cudaGetLastError();
     return MFC_ERR_ALLOC;
   }
+  if (g->kp.eta > 0.0 && cudaMalloc(&g->vel, sizeof(double) * (size_t)g->ndim * (size_t)cells) != cudaSuccess) {
+    cudaGetLastError();
+    mfc_free_grid(g);
+    return fail(MFC_ERR_ALLOC, "mfc_init_grid: allocation of the velocity arrays failed");
+  }
   g->kp.flag = g->d_flag;
   CK(cudaMemsetAsync(g->d_flag, 0, sizeof(int), g->stream));
   CK(cudaMemsetAsync(g->d_red, 0, 16, g->stream));
@@ -1075,6 +1197,7 @@ mfc_status mfc_free_grid(mfc_grid* g) {
   cudaStreamSynchronize(g->stream);
   cudaFree(g->q1);
   cudaFree(g->Lq);
+  cudaFree(g->vel);
   cudaFree(g->hq);
   cudaFree(g->hr);
   cudaFree(g->d_red);

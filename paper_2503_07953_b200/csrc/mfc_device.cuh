@@ -20,6 +20,7 @@ struct KP {
   double eps4;   // 4 * weno_eps (the smoothness indicators are carried scaled by 4)
   double alpha_floor;
   int clamp;
+  double eta;    // uniform shear viscosity of PAPER.md eq.(1); 0 = inviscid
   int kapila;    // 1: add K div(u) to the volume-fraction equations (two fluids)
   double gam[2]; // gamma_i and gamma_i pi_inf_i of the two fluids: rho_i c_i^2 = gamma_i p + gamma_i pi_inf_i (eq. 6)
   double gpi[2];

@@ -740,3 +740,54 @@ def test_weno_eps_below_the_product_form_range_is_refused(torch, mfc):
     with pytest.raises(mfc.MfcError) as e:
         mfc.Grid.from_case(make_case(1, 1, (16, 1, 1), W.BC_EXTRAP, eps=1e-80))
     assert e.value.status == mfc.MFC_ERR_ARG
+
+
+# ------------------------------------------------------------------ viscous terms (eta > 0)
+@pytest.mark.gpu
+@pytest.mark.parametrize("bc", [W.BC_PERIODIC, W.BC_EXTRAP])
+@pytest.mark.parametrize("ndim,nfluids,n", [(1, 2, (97, 1, 1)), (1, 1, (5, 1, 1)), (2, 2, (67, 35, 1)), (2, 3, (3, 2, 1)),
+                                            (3, 2, (33, 18, 11)), (3, 3, (40, 9, 13)), (3, 1, (16, 16, 16)), (3, 2, (2, 2, 2))])
+def test_rhs_rough_state_viscous(torch, mfc, ndim, nfluids, n, bc):
+    # eta sized so that the viscous rates are of the order of the inviscid ones on this rough state
+    case = replace(make_case(ndim, nfluids, n, bc), eta=3.0e3)
+    q = rough_state(case, 5 + ndim)
+    ref, noise = oracle_rhs_with_noise(case, q)
+    inviscid = O.Oracle(replace(case, eta=0.0)).rhs(q)
+    mom = slice(nfluids, nfluids + ndim)
+    if min(n[:ndim]) > 1:
+        assert np.abs(ref - inviscid)[mom].max() > 1e-2 * np.abs(ref[mom]).max()      # the terms are there
+    got = gpu_rhs(torch, mfc, case, q)
+    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None)
+    assert worst <= RHS_TOL, per
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("index,n,nsteps,eta", [(2, None, 100, 0.1), (3, 96, 100, 1e-3), (4, 40, 50, 0.05), (5, 32, 20, 0.05)])
+def test_rk3_steps_configs_viscous(torch, mfc, index, n, nsteps, eta):
+    case = replace(W.config(index, n=n), eta=eta)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    for s in range(nsteps):
+        dt_ref = orc.cfl_dt(ref, case.cfl)
+        orc.rk3_step(ref, dt_ref)
+        assert orc.bad == 0
+        g.rk3_step(qd, dt_ref)
+    g.check()
+    got = qd.cpu().numpy()
+    inviscid = W.initial_state(case)
+    assert np.isfinite(got).all()
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    g.close()
+    assert worst <= STEP_TOL, per
+
+
+@pytest.mark.gpu
+def test_viscous_refusals(torch, mfc):
+    with pytest.raises(mfc.MfcError):
+        mfc.Grid.from_case(replace(make_case(2, 1, (16, 16, 1), W.BC_EXTRAP), eta=-1.0))
+    from paper_2503_07953_b200 import slab as S
+    with pytest.raises(mfc.MfcError):
+        S.Slab(replace(make_case(3, 2, (16, 8, 12), W.BC_PERIODIC), eta=0.1))     # halos do not carry what the viscous stencil needs
