@@ -251,6 +251,34 @@ def config(index, n=None, seed=DEFAULT_SEED):
     raise ValueError("config index must be 1..5")
 
 
+def taylor_green(n=64, mach=0.1, reynolds=1600.0):
+    """The shape of the paper's viscous example (three-dimensional Taylor-Green vortex): single ideal gas on
+    the periodic box [0, 2 pi]^3, u = V0 (sin x cos y cos z, -cos x sin y cos z, 0),
+    p = p0 + rho0 V0^2/16 (cos 2x + cos 2y)(cos 2z + 2), rho = rho0; V0 = mach * sqrt(gamma p0/rho0), eta = rho0 V0 / reynolds
+    (reference length 1).  Closed form, no random numbers."""
+    L = 2.0 * np.pi
+    gamma, rho0, p0 = 1.4, 1.0, 1.0
+    v0 = mach * np.sqrt(gamma * p0 / rho0)
+    return Case("taylor_green_3d", 3, (n, n, n), (L / n,) * 3, 1, (gamma,), (0.0,), (_P,) * 3, (_P,) * 3, clamp=False,
+                nsteps=0, builder="taylor_green", eta=rho0 * v0 / reynolds, t_end=mach)
+
+
+def _build_taylor_green(case):
+    X, Y, Z = centres(case)
+    gamma, rho0, p0 = case.gamma[0], 1.0, 1.0
+    v0 = case.t_end * np.sqrt(gamma * p0 / rho0)  # t_end carries the Mach number of the case
+    shape3 = case.shape[1:]
+    u = v0 * np.sin(X) * np.cos(Y) * np.cos(Z)
+    v = -v0 * np.cos(X) * np.sin(Y) * np.cos(Z)
+    p = p0 + rho0 * v0 * v0 / 16.0 * (np.cos(2 * X) + np.cos(2 * Y)) * (np.cos(2 * Z) + 2.0)
+    rho = np.full(shape3, rho0)
+    return cons_from_prim(case, [rho], [np.broadcast_to(u, shape3), np.broadcast_to(v, shape3), 0.0],
+                          np.broadcast_to(p, shape3), [np.ones(shape3)])
+
+
+_BUILDERS["taylor_green"] = _build_taylor_green
+
+
 def initial_state(case):
     """q0 as a C-contiguous float64 array of shape case.shape."""
     return np.ascontiguousarray(_BUILDERS[case.builder](case))

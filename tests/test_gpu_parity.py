@@ -791,3 +791,31 @@ def test_viscous_refusals(torch, mfc):
     from paper_2503_07953_b200 import slab as S
     with pytest.raises(mfc.MfcError):
         S.Slab(replace(make_case(3, 2, (16, 8, 12), W.BC_PERIODIC), eta=0.1))     # halos do not carry what the viscous stencil needs
+
+
+@pytest.mark.gpu
+def test_taylor_green_vortex_viscous_steps(torch, mfc):
+    # the shape of the paper's viscous example: 40 RK3 steps at 32^3, Re = 100, against the oracle; the
+    # kinetic energy must go down at close to the closed-form initial rate (3/4) eta V0^2
+    case = W.taylor_green(32, mach=0.1, reynolds=100.0)
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    ke = lambda s: float((0.5 * (s[1:4] ** 2).sum(axis=0) / s[0]).mean())
+    ke0, t = ke(q), 0.0
+    for _ in range(40):
+        dt = orc.cfl_dt(ref, 0.5)
+        assert g.cfl_dt(qd, 0.5) == pytest.approx(dt, rel=1e-12)
+        orc.rk3_step(ref, dt)
+        g.rk3_step(qd, dt)
+        t += dt
+    g.check()
+    got = qd.cpu().numpy()
+    worst, per = rel_err(got, ref, 1, 3)
+    assert worst <= STEP_TOL, per
+    v0 = 0.1 * np.sqrt(1.4)
+    rate = (ke(got) - ke0) / t
+    assert rate == pytest.approx(-0.75 * case.eta * v0 * v0, rel=0.05)
+    g.close()

@@ -130,3 +130,24 @@ def test_rigid_motion_and_zero_viscosity_give_nothing():
     q, _, _ = state(case_nd(2, 12, bc=W.BC_EXTRAP), lambda X, Y, Z: (-2.0 * Y, 2.0 * X))   # rigid rotation: D = 0
     v = viscous_part(case_nd(2, 12, bc=W.BC_EXTRAP), q)
     assert np.abs(v[:, 0, 2:-2, 2:-2]).max() < 1e-11
+
+
+def test_taylor_green_vortex_dissipation_rate():
+    # the paper's viscous example shape.  For the divergence-free Taylor-Green field the viscous terms take
+    # kinetic energy out at the rate  -<u . div T> = eta <|curl u|^2> = (3/4) eta V0^2  (volume mean; closed form of the
+    # initial field).  The discrete rate converges to it at second order.
+    from dataclasses import replace
+    errs = []
+    for n in (16, 32):
+        case = W.taylor_green(n, mach=0.1, reynolds=100.0)
+        q = W.initial_state(case)
+        v = O.Oracle(case).rhs(q) - O.Oracle(replace(case, eta=0.0)).rhs(q)
+        rho = q[0]
+        u = q[1:4] / rho
+        rate = (u * v[1:4]).sum() / case.cells
+        v0 = 0.1 * np.sqrt(1.4)
+        exact = -0.75 * case.eta * v0 * v0
+        errs.append(abs(rate - exact) / abs(exact))
+        # total energy: the viscous work integrates to zero over the periodic box
+        assert abs(v[4].sum()) <= 1e-10 * np.abs(v[4]).sum()
+    assert errs[1] < 0.01 and 3.6 < errs[0] / errs[1] < 4.4, errs
