@@ -637,15 +637,27 @@ __global__ void __launch_bounds__(PB) viscous_kernel(const __grid_constant__ KP 
   ijk[0] = (int)(c % nx);
   ijk[1] = (int)((c / nx) % ny);
   ijk[2] = (int)(c / ((long long)nx * ny));
-  // mapped neighbour indices per direction (O1): nb[d][o+1], o = -1, 0, +1
+  // mapped neighbour indices per direction (O1): nb[d][o+1], o = -1, 0, +1 (the generic map only where n < 3)
   int nb[3][3];
 #pragma unroll
-  for (int d = 0; d < 3; ++d)
+  for (int d = 0; d < 3; ++d) {
+    const int n = kp.n[d], i = ijk[d];
+    nb[d][1] = i;
+    if (d < D && n >= 3) {
+      nb[d][0] = i > 0 ? i - 1 : (kp.bc_lo[d] == BC_PERIODIC ? n - 1 : 0);
+      nb[d][2] = i < n - 1 ? i + 1 : (kp.bc_hi[d] == BC_PERIODIC ? 0 : n - 1);
+    } else {
+      nb[d][0] = d < D ? ghost_index(i - 1, n, kp.bc_lo[d], kp.bc_hi[d]) : 0;
+      nb[d][2] = d < D ? ghost_index(i + 1, n, kp.bc_lo[d], kp.bc_hi[d]) : 0;
+    }
+  }
+  int rowbase[3][3];  // (k', j') -> offset of the row, 32-bit (fewer than 2^31 cells)
 #pragma unroll
-    for (int o = -1; o <= 1; ++o) nb[d][o + 1] = d < D ? ghost_index(ijk[d] + o, kp.n[d], kp.bc_lo[d], kp.bc_hi[d]) : 0;
+  for (int oz = 0; oz < 3; ++oz)
+#pragma unroll
+    for (int oy = 0; oy < 3; ++oy) rowbase[oz][oy] = (nb[2][oz] * ny + nb[1][oy]) * nx;
   auto U = [&](int m, const int* o) {  // velocity component m at offset o[3] from the cell
-    const long long t = ((long long)nb[2][o[2] + 1] * ny + nb[1][o[1] + 1]) * nx + nb[0][o[0] + 1];
-    return __ldg(vel + m * kp.ncells + t);
+    return __ldg(vel + m * kp.ncells + (rowbase[o[2] + 1][o[1] + 1] + nb[0][o[0] + 1]));
   };
   double acc[D + 1];
 #pragma unroll
