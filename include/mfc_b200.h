@@ -145,6 +145,11 @@ mfc_status mfc_rk3_steps(mfc_grid *g, double *q, double dt, int nsteps);
 mfc_status mfc_set_halo(mfc_grid *g, const double *halo_lo, const double *halo_hi);
 mfc_status mfc_pack_halo(mfc_grid *g, const double *q, int stage, double *send_lo, double *send_hi);
 mfc_status mfc_rk3_stage(mfc_grid *g, double *q, double dt, int stage);
+/* The same stage in two parts, so that the halo exchange can run while the first part computes: parts = 1 launches the
+ * sweeps of the directions before the last (they read no ghost layer of the last direction), parts = 2 the sweep of the
+ * last direction with the RK combination and clamp (it needs the halos), parts = 3 both (== mfc_rk3_stage).  Call part 1
+ * before part 2, on the same q and dt.  In 1-D part 1 is empty. */
+mfc_status mfc_rk3_stage_parts(mfc_grid *g, double *q, double dt, int stage, int parts);
 mfc_status mfc_stage_input(mfc_grid *g, const double *q, int stage, const double **state_out);
 
 /* dt = cfl / max_cells sum_d (|u_d| + c)/dx_d  with the frozen-alpha mixture sound speed

@@ -20,7 +20,7 @@ EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "m
            "mfc_rhs_dirs", "mfc_rk3_step", "mfc_rk3_steps", "mfc_cfl_dt", "mfc_check", "mfc_rhs_host",
            "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
            "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error", "mfc_set_halo", "mfc_rk3_stage",
-           "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64")
+           "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64", "mfc_rk3_stage_parts")
 
 
 KERNEL_CLASSES = ("prim", "sweep_x", "sweep_y", "sweep_z", "rk", "cfl")
@@ -80,6 +80,7 @@ def lib():
         L.mfc_last_error.restype = C.c_char_p
         L.mfc_set_halo.argtypes = [vp, dp, dp]
         L.mfc_rk3_stage.argtypes = [vp, dp, C.c_double, C.c_int]
+        L.mfc_rk3_stage_parts.argtypes = [vp, dp, C.c_double, C.c_int, C.c_int]
         L.mfc_stage_input.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_void_p)]
         L.mfc_pack_halo.argtypes = [vp, dp, C.c_int, dp, dp]
         L.mfc_measure_fp64.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -252,8 +253,9 @@ class Grid:
         hi = _dev_ptr(send_hi, send_hi.numel()) if send_hi is not None else None
         _ck(lib().mfc_pack_halo(self._h, _dev_ptr(q, self.count), int(stage), lo, hi))
 
-    def rk3_stage(self, q, dt, stage):
-        _ck(lib().mfc_rk3_stage(self._h, _dev_ptr(q, self.count), float(dt), int(stage)))
+    def rk3_stage(self, q, dt, stage, parts=3):
+        """parts: 1 = the sweeps before the last direction, 2 = the last sweep with the RK stage, 3 = both"""
+        _ck(lib().mfc_rk3_stage_parts(self._h, _dev_ptr(q, self.count), float(dt), int(stage), int(parts)))
 
     def stage_input_ptr(self, q, stage):
         """device address of the array stage `stage` sweeps (stage 1: q itself)"""

@@ -967,21 +967,30 @@ static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mas
 // One RK stage: L(qs) by the D sweeps, the last of which applies the stage combination and the clamp itself
 // (no separate RK kernel, the finished L never goes to HBM).  Stages 1 and 2 leave the new stage state in `work`
 // (where the partial L was), stage 3 writes q^{n+1} over q^n.
+// parts: bit 0 = the sweeps that do not touch the last direction (they need no halo of a slab), bit 1 = the last sweep,
+// which also applies the RK stage.  3 = the whole stage.
 template <int N, int D, int WV, int STAGE>
-static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, double* qn, double dt) {
+static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, double* qn, double dt, int parts = 3) {
   cudaError_t e;
   const bool visc = g->kp.eta > 0.0;
-  if (visc)
-    if ((e = launch_viscous<N, D>(g, qs, work)) != cudaSuccess) return e;
   if constexpr (D == 1) {
+    if (!(parts & 2)) return cudaSuccess;
+    if (visc)
+      if ((e = launch_viscous<N, D>(g, qs, work)) != cudaSuccess) return e;
     return visc ? launch_x<N, D, WV, true, STAGE>(g, qs, work, qn, dt) : launch_x<N, D, WV, false, STAGE>(g, qs, work, qn, dt);
   } else {
-    e = visc ? launch_x<N, D, WV, true, 0>(g, qs, work, nullptr, 0.0) : launch_x<N, D, WV, false, 0>(g, qs, work, nullptr, 0.0);
-    if (e != cudaSuccess) return e;
+    if (parts & 1) {
+      if (visc)
+        if ((e = launch_viscous<N, D>(g, qs, work)) != cudaSuccess) return e;
+      e = visc ? launch_x<N, D, WV, true, 0>(g, qs, work, nullptr, 0.0) : launch_x<N, D, WV, false, 0>(g, qs, work, nullptr, 0.0);
+      if (e != cudaSuccess) return e;
+      if constexpr (D == 3)
+        if ((e = launch_march<N, D, WV, 1, true, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
+    }
+    if (!(parts & 2)) return cudaSuccess;
     if constexpr (D == 2) {
       return launch_march<N, D, WV, 1, true, STAGE>(g, qs, work, qn, dt);
     } else {
-      if ((e = launch_march<N, D, WV, 1, true, 0>(g, qs, work, nullptr, 0.0)) != cudaSuccess) return e;
       return launch_march<N, D, WV, 2, true, STAGE>(g, qs, work, qn, dt);
     }
   }
@@ -1076,12 +1085,12 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
 #endif
 
 template <int N, int D, int WV>
-static cudaError_t launch_rk3_stage(mfc_grid* g, double* q, double dt, int stage) {
+static cudaError_t launch_rk3_stage(mfc_grid* g, double* q, double dt, int stage, int parts) {
   if constexpr (WV >= 3 && N != 2) return cudaErrorInvalidValue;
   else {
-    if (stage == 1) return launch_stage<N, D, WV, 1>(g, q, g->Lq, q, dt);
-    if (stage == 2) return launch_stage<N, D, WV, 2>(g, g->Lq, g->q1, q, dt);
-    return launch_stage<N, D, WV, 3>(g, g->q1, g->Lq, q, dt);
+    if (stage == 1) return launch_stage<N, D, WV, 1>(g, q, g->Lq, q, dt, parts);
+    if (stage == 2) return launch_stage<N, D, WV, 2>(g, g->Lq, g->q1, q, dt, parts);
+    return launch_stage<N, D, WV, 3>(g, g->q1, g->Lq, q, dt, parts);
   }
 }
 
@@ -1265,15 +1274,18 @@ mfc_status mfc_rk3_steps(mfc_grid* g, double* q, double dt, int nsteps) {
   return MFC_OK;
 }
 
-mfc_status mfc_rk3_stage(mfc_grid* g, double* q, double dt, int stage) {
+mfc_status mfc_rk3_stage_parts(mfc_grid* g, double* q, double dt, int stage, int parts) {
   if (!g || !q) return fail(MFC_ERR_ARG, "mfc_rk3_stage: NULL argument");
   if (stage < 1 || stage > 3) return fail(MFC_ERR_ARG, "mfc_rk3_stage: stage must be 1, 2 or 3");
+  if (parts < 1 || parts > 3) return fail(MFC_ERR_ARG, "mfc_rk3_stage_parts: parts must be 1, 2 or 3");
   if (!(dt == dt)) return fail(MFC_ERR_ARG, "mfc_rk3_stage: dt is NaN");
-  if (halo_missing(g)) return fail(MFC_ERR_ARG, "mfc_rk3_stage: MFC_BC_HALO without mfc_set_halo");
+  if ((parts & 2) && halo_missing(g)) return fail(MFC_ERR_ARG, "mfc_rk3_stage: MFC_BC_HALO without mfc_set_halo");
   if (mfc_status s = use_device(g)) return s;
-  CK(MFC_DISPATCH_W(g, (launch_rk3_stage<N, D, WV>(g, q, dt, stage))));
+  CK(MFC_DISPATCH_W(g, (launch_rk3_stage<N, D, WV>(g, q, dt, stage, parts))));
   return MFC_OK;
 }
+
+mfc_status mfc_rk3_stage(mfc_grid* g, double* q, double dt, int stage) { return mfc_rk3_stage_parts(g, q, dt, stage, 3); }
 
 mfc_status mfc_stage_input(mfc_grid* g, const double* q, int stage, const double** state_out) {
   if (!g || !q || !state_out) return fail(MFC_ERR_ARG, "mfc_stage_input: NULL argument");

@@ -4,7 +4,8 @@ The paper populates its buffer regions across processes by message passing (PAPE
 an ordinary handle of the C-ABI library whose last direction has MFC_BC_HALO on the ends that touch a neighbour:
 before every RHS evaluation the three layers next to each such end are packed (mfc_pack_halo, one strided
 device copy per end), exchanged with the neighbours (NCCL send/recv through torch.distributed; a device copy when the
-neighbour is the slab itself) and read by the sweep of that direction as its ghost cells.  Per RK3 step: three
+neighbour is the slab itself) and read by the sweep of that direction as its ghost cells; the sweeps of the other
+directions run while the transfer is in flight (mfc_rk3_stage_parts).  Per RK3 step: three
 exchanges of neq*3*plane doubles per end and one scalar MIN all-reduce for dt.  Everything else is the single-GPU path.
 
 This module is host plumbing only (partition, neighbours, buffers, the exchange); all arithmetic runs in the kernels.
@@ -52,15 +53,16 @@ def local_case(case, rank, world):
     return replace(case, n=tuple(n), bc_lo=tuple(lo), bc_hi=tuple(hi)), start, cnt
 
 
-def exchange(send_lo, send_hi, halo_lo, halo_hi, rank, below, above, dist=None, group=None):
+def exchange(send_lo, send_hi, halo_lo, halo_hi, rank, below, above, dist=None, group=None, wait=True):
     """send_lo -> below's halo_hi, send_hi -> above's halo_lo; receive halo_lo <- below's send_hi, halo_hi <- above's send_lo.
     A neighbour equal to `rank` (one slab, periodic) is a local copy.  Posting order: with two slabs on a periodic domain both
-    messages go to the same peer; it sends (send_lo, send_hi) in that order, so the receives are posted (halo_hi, halo_lo)."""
+    messages go to the same peer; it sends (send_lo, send_hi) in that order, so the receives are posted (halo_hi, halo_lo).
+    wait=False returns the pending work handles (the caller waits on them before the sweep that reads the halos)."""
     ops = []
     if below == rank and above == rank:
         halo_lo.copy_(send_hi)
         halo_hi.copy_(send_lo)
-        return
+        return []
     if below is not None:
         ops.append(dist.P2POp(dist.isend, send_lo, below, group))
     if above is not None:
@@ -69,9 +71,12 @@ def exchange(send_lo, send_hi, halo_lo, halo_hi, rank, below, above, dist=None, 
         ops.append(dist.P2POp(dist.irecv, halo_hi, above, group))
     if below is not None:
         ops.append(dist.P2POp(dist.irecv, halo_lo, below, group))
-    if ops:
-        for w in dist.batch_isend_irecv(ops):
+    works = dist.batch_isend_irecv(ops) if ops else []
+    if wait:
+        for w in works:
             w.wait()
+        return []
+    return works
 
 
 class Slab:
@@ -99,25 +104,32 @@ class Slab:
         if self.send_lo is not None or self.send_hi is not None:
             self.grid.pack_halo(q, stage, self.send_lo, self.send_hi)
 
-    def refresh(self, q, stage=1):
-        """ghost layers of the state that stage `stage` sweeps (stage 1: q)"""
+    def refresh(self, q, stage=1, wait=True):
+        """ghost layers of the state that stage `stage` sweeps (stage 1: q).  wait=False: returns the pending transfers"""
         if self.below is None and self.above is None:
-            return
+            return []
         import torch
         self.pack(q, stage)
         if not (self.below == self.rank and self.above == self.rank):
             torch.cuda.current_stream().synchronize()  # the packed buffers must be complete before NCCL reads them on its stream
-        exchange(self.send_lo, self.send_hi, self.halo_lo, self.halo_hi, self.rank, self.below, self.above, self.dist, self.group)
+        works = exchange(self.send_lo, self.send_hi, self.halo_lo, self.halo_hi, self.rank, self.below, self.above,
+                         self.dist, self.group, wait)
         self.exchanges += 1
+        return works
 
     def rhs(self, q, out):
         self.refresh(q, 1)
         self.grid.rhs(q, out)
 
     def rk3_step(self, q, dt):
+        """per stage: start the halo exchange, run the sweeps that need no halo while it is in flight, wait, run the last
+        sweep (which reads the halos and applies the RK stage)"""
         for stage in (1, 2, 3):
-            self.refresh(q, stage)
-            self.grid.rk3_stage(q, dt, stage)
+            works = self.refresh(q, stage, wait=False)
+            self.grid.rk3_stage(q, dt, stage, parts=1)
+            for w in works:
+                w.wait()
+            self.grid.rk3_stage(q, dt, stage, parts=2)
 
     def cfl_dt(self, q, cfl):
         """global dt: the minimum over slabs of the local one (one scalar all-reduce)"""
