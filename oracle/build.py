@@ -17,9 +17,11 @@ DEPS = SRC + [os.path.join(HERE, "mfc_oracle.hpp")]
 def build(force: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
         return LIB
+    tmp = LIB + ".tmp.%d" % os.getpid()  # complete before it takes the library's name (several processes may build at once)
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
-           "-Wall", "-Wextra", "-Wno-maybe-uninitialized", "-o", LIB] + SRC
+           "-Wall", "-Wextra", "-Wno-maybe-uninitialized", "-o", tmp] + SRC
     subprocess.check_call(cmd)
+    os.replace(tmp, LIB)
     return LIB
 
 

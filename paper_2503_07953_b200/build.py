@@ -18,12 +18,27 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std
          "--fmad=true", "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
 
+def _fresh() -> bool:
+    return os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
+    if not force and _fresh():
         return LIB
-    extra = os.environ.get("MFC_B200_NVCC_EXTRA", "").split()
-    cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
-    subprocess.check_call(cmd)
+    # several ranks of one job may get here together: one compiles (into a temporary, renamed when complete), the
+    # others wait on the lock and find the library fresh
+    import fcntl
+    with open(LIB + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if force or not _fresh():
+                extra = os.environ.get("MFC_B200_NVCC_EXTRA", "").split()
+                tmp = LIB + ".tmp.%d" % os.getpid()
+                cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC
+                subprocess.check_call(cmd)
+                os.replace(tmp, LIB)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return LIB
 
 
