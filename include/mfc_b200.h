@@ -4,7 +4,9 @@
  * model with stiffened-gas EOS — conservative->primitive conversion, WENO5-JS reconstruction of the
  * primitives, HLLC fluxes, flux divergence and the alpha_i div(u) source — and advances it by SSP-RK3.
  * Every step runs in hand-written fp64 CUDA kernels for sm_100a; there is NO CPU fallback: if no CUDA
- * device is usable every call returns MFC_ERR_CUDA.
+ * device is usable every call returns MFC_ERR_CUDA.  Options of mfc_params beyond that path: mapped or
+ * WENO-Z weights (weno), the Kapila K div(u) term (model), the viscous stress (eta); and MFC_BC_HALO with
+ * mfc_set_halo / mfc_pack_halo / mfc_rk3_stage(_parts) for slabs of one domain on several GPUs.
  *
  * Citations are PAPER.md lines (section / equation).  Readings of points the paper leaves open carry the
  * A-numbers of DESIGN.md §3.
@@ -22,7 +24,8 @@
  * OWNERSHIP: the caller owns q, w, rhs.  "device" pointers are CUDA device pointers valid on the
  * handle's device (e.g. torch.Tensor.data_ptr()), 8-byte aligned; "host" pointers are ordinary host
  * memory (pinned memory makes the *_host calls faster but is not required).  The handle owns its scratch
- * (two state-sized arrays, a few bytes of reduction/flag storage) and never frees caller memory.
+ * (two state-sized arrays, D cell-sized arrays of velocities when eta > 0, a few bytes of reduction/flag
+ * storage) and never frees caller memory.
  *
  * STREAMS: every kernel is enqueued on the stream given at mfc_init_grid (NULL = the legacy default
  * stream).  Calls marked "async" return after enqueueing.  Calls marked "syncs" wait for that stream.
