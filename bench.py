@@ -256,20 +256,25 @@ def main():
     for _ in range(args.warmup):
         advance(qd, case.cfl, 1)
     g.check()
-    sampler = ClockSampler(local_rank)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    l0 = g.launch_count()
-    barrier()
-    sampler.start()
-    ev0.record()
-    advance(qd, case.cfl, args.steps)
-    ev1.record()
-    torch.cuda.synchronize()
-    clocks = sampler.stop()
-    barrier()
-    launches = g.launch_count() - l0
-    ms = reduce_max_ms(ev0.elapsed_time(ev1), world)
-    g.check()
+    bad_reasons = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+    for attempt in (1, 2):  # a run that saw a thermal / hardware slowdown is re-measured once (sw_power_cap is kept and noted)
+        sampler = ClockSampler(local_rank)
+        l0 = g.launch_count()
+        barrier()
+        sampler.start()
+        ev0.record()
+        advance(qd, case.cfl, args.steps)
+        ev1.record()
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        barrier()
+        launches = g.launch_count() - l0
+        ms = reduce_max_ms(ev0.elapsed_time(ev1), world)
+        g.check()
+        clocks["attempt"] = attempt
+        if not (bad_reasons & set(clocks.get("reasons") or [])):
+            break
     value = grind_ns(ms, args.steps, cells, neq, world)
 
     # ---- per-kernel device times (CUDA events around every launch, on the launching stream) for the roofline
