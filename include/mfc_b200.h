@@ -173,8 +173,11 @@ mfc_status mfc_rk3_steps_host(mfc_grid *g, double *q_host, double dt, int nsteps
 
 /* Adaptive stepping, all on the device timeline: nsteps times { dt = CFL step of the current state (as
  * mfc_cfl_dt); one RK3 step of size dt }.  *t_elapsed_host (HOST, may be NULL) receives the sum of the dt.
- * mfc_advance: q device, syncs once per step (the 8-byte dt read-back).  mfc_advance_host: q_host HOST,
- * copied in before and out after the nsteps steps. */
+ * dt never leaves the device: a one-thread kernel turns the reduction's maximum into dt and adds it to the elapsed time,
+ * the RK stages read it from device memory — same kernels and IEEE arithmetic as the caller's own loop of mfc_cfl_dt +
+ * mfc_rk3_step (bit-identical states and elapsed time), without a host round trip per step.  Both calls synchronise once,
+ * at the end, and then report the sticky non-physical flag (a state that turns non-physical in step k is still stepped to
+ * the end).  mfc_advance: q device.  mfc_advance_host: q_host HOST, copied in before and out after the nsteps steps. */
 mfc_status mfc_advance(mfc_grid *g, double *q, double cfl, int nsteps, double *t_elapsed_host);
 mfc_status mfc_advance_host(mfc_grid *g, double *q_host, double cfl, int nsteps, double *t_elapsed_host);
 

@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
           qnc[v] = qnn[v * kp.ncells + off];
           qsc[v] = STAGE >= 2 ? __ldg(q + v * kp.ncells + off) : 0.0;
         }
-        rk_cell<N, D, STAGE>(kp, dt, qnc, qsc, r);
+        rk_cell<N, D, STAGE>(kp, kp.dt_dev ? __ldg(kp.dt_dev) : dt, qnc, qsc, r);
       }
       double* out = STAGE == 3 ? qnn : rhs;
 #pragma unroll
@@ -510,7 +510,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
             qsc[2 * h + 1 < NEQ ? 2 * h + 1 : 0] = b.y;
           }
         }
-        rk_cell<N, D, STAGE>(kp, dt, qnc, qsc, r);
+        rk_cell<N, D, STAGE>(kp, kp.dt_dev ? __ldg(kp.dt_dev) : dt, qnc, qsc, r);
       }
       double* out = STAGE == 3 ? qnn : rhs;
 #pragma unroll
@@ -576,6 +576,16 @@ __global__ void __launch_bounds__(PB) cfl_kernel(const __grid_constant__ KP kp, 
     if (threadIdx.x == 0 && smax > 0.0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(smax));
   }
   if (bad) *kp.flag = 1;
+}
+
+// dt = cfl / (maximum left by cfl_kernel), t += dt, and the maximum is cleared for the next reduction: keeps the time
+// step on the device so that mfc_advance needs no host round trip per step.  IEEE operations, the host's arithmetic.
+__global__ void dt_kernel(unsigned long long* smax_bits, double cfl, double* dt_t) {
+  const double smax = __longlong_as_double((long long)*smax_bits);
+  const double dt = __ddiv_rn(cfl, smax);
+  dt_t[0] = dt;
+  dt_t[1] = __dadd_rn(dt_t[1], dt);
+  *smax_bits = 0ull;
 }
 
 // ------------------------------------------------------------------------------------------------ unit entry points
@@ -748,6 +758,7 @@ struct mfc_grid {
   double* hr = nullptr;
   unsigned long long* d_red = nullptr;  // [0] = smax bits
   int* d_flag = nullptr;
+  double* d_dt = nullptr;               // [0] dt of the step in flight, [1] elapsed time (mfc_advance)
   unsigned* d_xnext = nullptr;          // two work counters of sweep_x, used alternately (each launch zeroes the other)
   int xparity = 0;
   int xchunk = 0;                       // items per chunk (0 = default)
@@ -1192,6 +1203,7 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   cudaError_t e;
   if ((e = cudaMalloc(&g->q1, bytes)) != cudaSuccess || (e = cudaMalloc(&g->Lq, bytes)) != cudaSuccess ||
       (e = cudaMalloc(&g->d_red, 16)) != cudaSuccess || (e = cudaMalloc(&g->d_flag, sizeof(int))) != cudaSuccess ||
+      (e = cudaMalloc(&g->d_dt, 2 * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&g->d_xnext, 2 * sizeof(unsigned))) != cudaSuccess ||
       (e = cudaMallocHost(&g->h_red, 16)) != cudaSuccess) {
     mfc_free_grid(g);
@@ -1223,6 +1235,7 @@ mfc_status mfc_free_grid(mfc_grid* g) {
   cudaFree(g->hr);
   cudaFree(g->d_red);
   cudaFree(g->d_flag);
+  cudaFree(g->d_dt);
   cudaFree(g->d_xnext);
   if (g->h_red) cudaFreeHost(g->h_red);
   drain_profile(g);
@@ -1391,16 +1404,29 @@ mfc_status mfc_rk3_steps_host(mfc_grid* g, double* q_host, double dt, int nsteps
   return MFC_OK;
 }
 
+// CFL + RK3 per step, all on the device: the reduction leaves max_cells sum_d (|u_d|+c)/dx_d, dt_kernel turns it into dt
+// and adds it to the elapsed time, the RK stages read dt from device memory.  One host synchronisation at the end, which
+// also reports the sticky non-physical flag.  Same kernels and arithmetic as the caller's loop of mfc_cfl_dt + mfc_rk3_step.
 static mfc_status advance_impl(mfc_grid* g, double* q, double cfl, int nsteps, double* t_out) {
-  double t = 0.0;
+  CK(cudaMemsetAsync(g->d_dt, 0, 2 * sizeof(double), g->stream));
+  CK(cudaMemsetAsync(g->d_red, 0, 8, g->stream));
   for (int s = 0; s < nsteps; ++s) {
-    double dt = 0.0;
-    if (mfc_status st = mfc_cfl_dt(g, q, cfl, &dt)) return st;
-    CK(MFC_DISPATCH_W(g, (launch_rk3<N, D, WV>(g, q, dt))));
-    t += dt;
+    CK(MFC_DISPATCH(g, (launch_cfl<N, D>(g, q))));
+    {
+      Scope sc(g, MFC_K_CFL);
+      dt_kernel<<<1, 1, 0, g->stream>>>(g->d_red, cfl, g->d_dt);
+    }
+    CK(cudaGetLastError());
+    g->kp.dt_dev = g->d_dt;
+    const cudaError_t e = MFC_DISPATCH_W(g, (launch_rk3<N, D, WV>(g, q, 0.0)));
+    g->kp.dt_dev = nullptr;
+    CK(e);
   }
-  if (t_out) *t_out = t;
-  return MFC_OK;
+  CK(cudaMemcpyAsync(&g->h_red[0], g->d_dt + 1, 8, cudaMemcpyDeviceToHost, g->stream));
+  g->h_red[1] = 0;
+  const mfc_status st = read_flag_and_sync(g, false);
+  if (t_out) std::memcpy(t_out, &g->h_red[0], 8);
+  return st;
 }
 
 mfc_status mfc_advance(mfc_grid* g, double* q, double cfl, int nsteps, double* t_elapsed_host) {

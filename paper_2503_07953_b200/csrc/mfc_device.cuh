@@ -25,6 +25,7 @@ struct KP {
   double gam[2]; // gamma_i and gamma_i pi_inf_i of the two fluids: rho_i c_i^2 = gamma_i p + gamma_i pi_inf_i (eq. 6)
   double gpi[2];
   int* flag;     // sticky non-physical flag (A19)
+  const double* dt_dev;  // if not NULL the RK stages take dt from here (mfc_advance keeps dt on the device) instead of the argument
   // BC_HALO on the last direction (slab decomposition): the three ghost layers beyond each end, [neq][3][plane]
   const double* halo_lo;
   const double* halo_hi;
