@@ -277,6 +277,24 @@ def main():
             break
     value = grind_ns(ms, args.steps, cells, neq, world)
 
+    # ---- mfc_rhs alone (SURVEY §8(d) metric (i)): x, y, z sweeps without the RK stage, rhs written to its own array
+    rhs_only = None
+    if slab is None:
+        rd = torch.empty_like(qd)
+        for _ in range(3):
+            g.rhs(qd, rd)
+        n_rhs = max(3, min(3 * args.steps, 30))
+        torch.cuda.synchronize()
+        ev0.record()
+        for _ in range(n_rhs):
+            g.rhs(qd, rd)
+        ev1.record()
+        torch.cuda.synchronize()
+        r_ms = reduce_max_ms(ev0.elapsed_time(ev1), world) / n_rhs
+        rhs_only = {"value": r_ms * 1e6 / (cells * neq), "unit": "ns/cell/eqn/rhs_eval", "ms_per_rhs": r_ms, "evals": n_rhs,
+                    "call": "mfc_rhs"}
+        del rd
+
     # ---- per-kernel device times (CUDA events around every launch, on the launching stream) for the roofline
     g.set_profiling(True)
     advance(qd, case.cfl, args.steps)
@@ -352,7 +370,7 @@ def main():
                    "l2": "inputs larger than L2 (state array %.0f MB vs 126 MB L2)" % (8e-6 * neq * cells) if 8 * neq * cells > 3e8
                    else "working set fits L2: latency/L2-bound configuration, roofline target does not apply"},
         "cell_updates_per_s": cells * world * args.steps / (ms * 1e-3),
-        "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roofline,
+        "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "rhs_only": rhs_only, "roofline": roofline,
         "paper_context": "PAPER.md:720-726 Table 1 (other hardware, whole step): GH200 0.32, H100 SXM 0.38, A100 0.62 ns",
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
