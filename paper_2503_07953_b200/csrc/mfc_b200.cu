@@ -133,6 +133,7 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
   const double idx = kp.inv_dx[0];
   const int lo = kp.bc_lo[0], hi = kp.bc_hi[0];
   bool bad = false;
+  const double dtv = (STAGE >= 1 && kp.dt_dev) ? __ldg(kp.dt_dev) : dt;  // mfc_advance keeps dt on the device; read it once
   int it1 = 0;  // end of the current chunk of items
 
   auto set_item = [&](XCursor& c) {
@@ -257,7 +258,7 @@ __global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_const
           qnc[v] = qnn[v * kp.ncells + off];
           qsc[v] = STAGE >= 2 ? __ldg(q + v * kp.ncells + off) : 0.0;
         }
-        rk_cell<N, D, STAGE>(kp, kp.dt_dev ? __ldg(kp.dt_dev) : dt, qnc, qsc, r);
+        rk_cell<N, D, STAGE>(kp, dtv, qnc, qsc, r);
       }
       double* out = STAGE == 3 ? qnn : rhs;
 #pragma unroll
@@ -353,6 +354,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
   };
 #define RG(slot, v) (*elem((slot) * SLOT, (v)))
   bool bad = false;
+  const double dtv = (STAGE >= 1 && kp.dt_dev) ? __ldg(kp.dt_dev) : dt;  // mfc_advance keeps dt on the device; read it once
   double qn[NEQ];
   auto loadq = [&](int off) {
 #pragma unroll
@@ -510,7 +512,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
             qsc[2 * h + 1 < NEQ ? 2 * h + 1 : 0] = b.y;
           }
         }
-        rk_cell<N, D, STAGE>(kp, kp.dt_dev ? __ldg(kp.dt_dev) : dt, qnc, qsc, r);
+        rk_cell<N, D, STAGE>(kp, dtv, qnc, qsc, r);
       }
       double* out = STAGE == 3 ? qnn : rhs;
 #pragma unroll
