@@ -827,3 +827,11 @@ def test_taylor_green_vortex_viscous_steps(torch, mfc):
     rate = (ke(got) - ke0) / t
     assert rate == pytest.approx(-0.75 * case.eta * v0 * v0, rel=0.05)
     g.close()
+
+
+@pytest.mark.gpu
+def test_fp64_probe_reports_plausible_rates(torch, mfc):
+    # mfc_measure_fp64 (bench.py's measured roofline denominator): the two-operand DFMA rate lies between half and all of
+    # the derived peak of a B200, and three distinct register operands cost what DESIGN.md §8 says (about 2/3 of it)
+    a, b = mfc.measure_fp64(0)
+    assert 15.0 < a < 40.0 and 0.55 < b / a < 0.85, (a, b)
