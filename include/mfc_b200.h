@@ -122,7 +122,8 @@ mfc_status mfc_prim_from_cons(mfc_grid *g, const double *q, double *w);
 mfc_status mfc_rhs(mfc_grid *g, const double *q, double *rhs);
 
 /* As mfc_rhs but only the directions whose bit is set in dir_mask (bit d = direction d) contribute;
- * cells keep 0 from the other directions.  Exists so that each directional sweep can be tested alone. */
+ * cells keep 0 from the other directions.  The viscous rates (eta > 0) are part of the result only for dir_mask == 7,
+ * whatever the number of dimensions.  Exists so that each directional sweep can be tested alone. */
 mfc_status mfc_rhs_dirs(mfc_grid *g, const double *q, double *rhs, int dir_mask);
 
 /* One SSP-RK3 step of size dt (the three-stage formula), in place on q, with the A10

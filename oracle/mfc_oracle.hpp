@@ -19,9 +19,10 @@
 // closed form (O2); WENO linear/closed-form/ENO/mirror/order-5 (O3); HLLC
 // consistency, upwinding, stationary contact, mirror (O4); Sod and water/air
 // exact Riemann solutions, uniform-state, conservation, interface equilibrium,
-// alpha==1 (O2-O6).  cfl_dt (A9) and the clamp (A10) are defined by
-// BASELINE.json only, not by the paper: "parity unpinned" beyond their
-// closed-form definition tests.
+// alpha==1 (O2-O6); third-order convergence in dt and the amplification polynomial
+// 1 + z + z^2/2 + z^3/6 of rk3_step (O6, tests/test_oracle_rk3.py).  cfl_dt (A9) and
+// the clamp (A10) are defined by BASELINE.json only, not by the paper: "parity
+// unpinned" beyond their closed-form definition tests.
 //
 // Everything is a template on the scalar T so that the same text gives the
 // fp64 oracle, a long double adjudicator and an operation-counting build.
@@ -43,6 +44,13 @@ enum { BC_PERIODIC = 0, BC_EXTRAP = 1 };
 // MODEL_KAPILA: ... = K_i div(u) with eq.(5), two fluids.
 enum { MODEL_ALLAIRE = 0, MODEL_KAPILA = 1 };
 enum { RECON_PIECEWISE_CONSTANT = 1, RECON_WENO5_JS = 5, RECON_WENO5_M = 6, RECON_WENO5_Z = 7 };
+// FORM_DIFFERENCE: O3 and O4 evaluated as DESIGN.md readings N2 / N3 write them (deviations from the cell value in first
+// differences; star-state jump with chi - 1 formed directly) — what every parity bar is measured against.
+// FORM_TEXTBOOK: the same definitions typed as the paper prints them: f = sum_r omega_r f^(r) with the
+// Jiang-Shu candidate polynomials, F = F_K + S_K (q*_K - q_K) with q*_K formed first (668).  A second,
+// independent evaluation of the same mathematics: tests use it to show that the CUDA path agrees with the paper's text as
+// closely as that text's own fp64 rounding allows, whatever form the first oracle is written in.
+enum { FORM_DIFFERENCE = 0, FORM_TEXTBOOK = 1 };
 
 // generic helpers so that T may be double, long double or the counting type
 template <class T> inline T o_sqrt(const T& x) { using std::sqrt; return sqrt(x); }
@@ -67,6 +75,7 @@ struct Params {
   int recon = RECON_WENO5_JS;
   int model = MODEL_ALLAIRE;
   T eta = T(0);            // uniform shear viscosity of eq.(1) (A22); 0 = inviscid
+  int form = FORM_DIFFERENCE;  // evaluation form of O3 / O4 (WENO5-JS and HLLC): readings N2, N3 or the textbook text
 
   int neq() const { return 2 * nfluids + ndim + 1; }  // PAPER.md:704 "two advected species (8 PDEs)" in 3D
   std::size_t cells() const { return std::size_t(n[0]) * n[1] * n[2]; }
@@ -314,6 +323,99 @@ int hllc_face(const Params<T>& P, int dir, const T* wL, const T* wR, T* F, T* uf
   return bad;
 }
 
+// O3, textbook form (f = sum_r omega_r f^(r); Jiang-Shu candidates and indicators, A3).  Same inputs and
+// outputs as weno5_js.
+template <class T>
+void weno5_js_textbook(const T& a, const T& b, const T& c, const T& d, const T& e, const T& eps, T* left, T* right) {
+  const T c1312 = o_ratio<T>(13, 12), c14 = o_ratio<T>(1, 4);
+  T t0 = a - T(2) * b + c, t1 = b - T(2) * c + d, t2 = c - T(2) * d + e;
+  T s0 = a - T(4) * b + T(3) * c, s1 = b - d, s2 = T(3) * c - T(4) * d + e;
+  T b0 = c1312 * (t0 * t0) + c14 * (s0 * s0);
+  T b1 = c1312 * (t1 * t1) + c14 * (s1 * s1);
+  T b2 = c1312 * (t2 * t2) + c14 * (s2 * s2);
+  {  // left-biased value at i+1/2: candidates of stencils (i-2..i), (i-1..i+1), (i..i+2), ideal weights (1/10, 6/10, 3/10)
+    T p0 = (T(2) * a - T(7) * b + T(11) * c) / T(6);
+    T p1 = (T(5) * c - b + T(2) * d) / T(6);
+    T p2 = (T(2) * c + T(5) * d - e) / T(6);
+    T a0 = o_ratio<T>(1, 10) / ((b0 + eps) * (b0 + eps));
+    T a1 = o_ratio<T>(6, 10) / ((b1 + eps) * (b1 + eps));
+    T a2 = o_ratio<T>(3, 10) / ((b2 + eps) * (b2 + eps));
+    T s = a0 + a1 + a2;
+    *left = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+  }
+  {  // right-biased value at i-1/2: the mirror image, ideal weights (3/10, 6/10, 1/10), same indicators
+    T p0 = (T(5) * b - a + T(2) * c) / T(6);
+    T p1 = (T(2) * b + T(5) * c - d) / T(6);
+    T p2 = (T(11) * c - T(7) * d + T(2) * e) / T(6);
+    T a0 = o_ratio<T>(3, 10) / ((b0 + eps) * (b0 + eps));
+    T a1 = o_ratio<T>(6, 10) / ((b1 + eps) * (b1 + eps));
+    T a2 = o_ratio<T>(1, 10) / ((b2 + eps) * (b2 + eps));
+    T s = a0 + a1 + a2;
+    *right = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+  }
+}
+
+// O4, textbook form: the star state q*_K of PAPER.md:668 is formed first (alpha_i carried like a passive density, A7) and
+// the flux is F_K + S_K (q*_K - q_K).  Same inputs, outputs, wave speeds and selection as hllc_face.
+template <class T>
+int hllc_face_textbook(const Params<T>& P, int dir, const T* wL, const T* wR, T* F, T* uf) {
+  const int N = P.nfluids, D = P.ndim, neq = P.neq();
+  const T* w[2] = {wL, wR};
+  T rho[2], Gam[2], Pi[2], E[2], c[2], un[2], p[2];
+  int bad = 0;
+  for (int K = 0; K < 2; ++K) {
+    rho[K] = T(0); Gam[K] = T(0); Pi[K] = T(0);
+    for (int i = 0; i < N; ++i) rho[K] = rho[K] + w[K][P.i_arho(i)];
+    for (int i = 0; i < N; ++i) {
+      Gam[K] = Gam[K] + w[K][P.i_alpha(i)] * P.G(i);
+      Pi[K] = Pi[K] + w[K][P.i_alpha(i)] * P.P(i);
+    }
+    T usq = T(0);
+    for (int d = 0; d < D; ++d) usq = usq + w[K][P.i_mom(d)] * w[K][P.i_mom(d)];
+    p[K] = w[K][P.i_E()];
+    un[K] = w[K][P.i_mom(dir)];
+    E[K] = Gam[K] * p[K] + Pi[K] + (T(0.5) * rho[K]) * usq;
+    T c2 = sound_speed_sq(Gam[K], Pi[K], p[K], rho[K]);
+    if (!(rho[K] > T(0)) || !(c2 > T(0))) bad = 1;
+    c[K] = o_sqrt(c2);
+  }
+  const T SL = o_min(un[0] - c[0], un[1] - c[1]);
+  const T SR = o_max(un[0] + c[0], un[1] + c[1]);
+  const T Sstar = (p[1] - p[0] + rho[0] * un[0] * (SL - un[0]) - rho[1] * un[1] * (SR - un[1])) /
+                  (rho[0] * (SL - un[0]) - rho[1] * (SR - un[1]));
+  auto side_flux = [&](int K, bool star, const T& SK) {
+    const T chi = star ? (SK - un[K]) / (SK - Sstar) : T(1);
+    for (int v = 0; v < neq; ++v) F[v] = T(0);
+    for (int i = 0; i < N; ++i) {
+      T qv = w[K][P.i_arho(i)];
+      F[P.i_arho(i)] = qv * un[K];
+      if (star) F[P.i_arho(i)] = F[P.i_arho(i)] + SK * (chi * qv - qv);
+      T av = w[K][P.i_alpha(i)];
+      F[P.i_alpha(i)] = av * un[K];
+      if (star) F[P.i_alpha(i)] = F[P.i_alpha(i)] + SK * (chi * av - av);  // A7
+    }
+    for (int d = 0; d < D; ++d) {
+      T qv = rho[K] * w[K][P.i_mom(d)];
+      F[P.i_mom(d)] = qv * un[K] + (d == dir ? p[K] : T(0));
+      if (star) {
+        T qs = (d == dir) ? chi * rho[K] * Sstar : chi * qv;
+        F[P.i_mom(d)] = F[P.i_mom(d)] + SK * (qs - qv);
+      }
+    }
+    F[P.i_E()] = (E[K] + p[K]) * un[K];
+    if (star) {
+      T Es = chi * (E[K] + (Sstar - un[K]) * (rho[K] * Sstar + p[K] / (SK - un[K])));
+      F[P.i_E()] = F[P.i_E()] + SK * (Es - E[K]);
+    }
+    *uf = star ? un[K] + SK * (chi - T(1)) : un[K];  // HLLC flux of a unit scalar (A7)
+  };
+  if (SL >= T(0)) side_flux(0, false, SL);  // first match in the printed order (A8)
+  else if (Sstar >= T(0)) side_flux(0, true, SL);
+  else if (SR > T(0)) side_flux(1, true, SR);
+  else side_flux(1, false, SR);
+  return bad;
+}
+
 // A10: positivity / volume-fraction clamp applied to one cell after each RK stage.
 template <class T>
 void clamp_cell(const Params<T>& P, T* q) {
@@ -383,7 +485,9 @@ struct Solver {
           for (int v = 0; v < neq; ++v) {
             const T* c = &wl[std::size_t(i + 3) * neq + v];
             T l, r;
-            if (P.recon == RECON_WENO5_JS) {
+            if (P.recon == RECON_WENO5_JS && P.form == FORM_TEXTBOOK) {
+              weno5_js_textbook(c[-2 * neq], c[-neq], c[0], c[neq], c[2 * neq], P.weno_eps, &l, &r);
+            } else if (P.recon == RECON_WENO5_JS) {
               weno5_js(c[-2 * neq], c[-neq], c[0], c[neq], c[2 * neq], P.weno_eps, &l, &r);
             } else if (P.recon == RECON_WENO5_M || P.recon == RECON_WENO5_Z) {
               weno5(P.recon, c[-2 * neq], c[-neq], c[0], c[neq], c[2 * neq], P.weno_eps, &l, &r);
@@ -396,8 +500,11 @@ struct Solver {
         }
         // faces f = i+1/2, i = -1..n-1: left state from cell i, right state from cell i+1
         for (int i = -1; i < n; ++i)
-          bad += hllc_face(P, dir, &WL[std::size_t(i + 1) * neq], &WR[std::size_t(i + 2) * neq],
-                           &Ff[std::size_t(i + 1) * neq], &uf[i + 1]);
+          bad += P.form == FORM_TEXTBOOK
+                     ? hllc_face_textbook(P, dir, &WL[std::size_t(i + 1) * neq], &WR[std::size_t(i + 2) * neq],
+                                          &Ff[std::size_t(i + 1) * neq], &uf[i + 1])
+                     : hllc_face(P, dir, &WL[std::size_t(i + 1) * neq], &WR[std::size_t(i + 2) * neq],
+                                 &Ff[std::size_t(i + 1) * neq], &uf[i + 1]);
         // eq.(10): flux difference and the alpha_i div(u) source with the cell-centre alpha_i
         for (int i = 0; i < n; ++i) {
           ijk[dir] = i;

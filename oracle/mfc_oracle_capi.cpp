@@ -28,6 +28,7 @@ typedef struct {
   int recon;
   int model;
   double eta;
+  int form;  /* FORM_DIFFERENCE (0) or FORM_TEXTBOOK (1) */
 } oracle_params;
 
 }  // extern "C"
@@ -55,6 +56,7 @@ Params<T> convert(const oracle_params* p) {
   P.recon = p->recon;
   P.model = p->model;
   P.eta = T(p->eta);
+  P.form = p->form;
   P.derive();
   return P;
 }

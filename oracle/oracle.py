@@ -23,7 +23,8 @@ class OracleParams(C.Structure):
     _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("dx", C.c_double * 3), ("nfluids", C.c_int),
                 ("gamma", C.c_double * _MAXF), ("pi_inf", C.c_double * _MAXF),
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
-                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("recon", C.c_int), ("model", C.c_int), ("eta", C.c_double)]
+                ("weno_eps", C.c_double), ("alpha_floor", C.c_double), ("clamp", C.c_int), ("recon", C.c_int), ("model", C.c_int), ("eta", C.c_double),
+                ("form", C.c_int)]
 
 
 _lib = None
@@ -91,9 +92,12 @@ def make_params(case, recon=None):
 class Oracle:
     """The five operations of include/mfc_b200.h on host numpy arrays (SoA, x fastest)."""
 
-    def __init__(self, case, recon=None):
+    def __init__(self, case, recon=None, form="difference"):
+        """form: "difference" (readings N2/N3, what the parity bars are measured against) or "textbook" (O3 and O4 typed
+        as PAPER.md:163 / 197 print them) — mfc_oracle.hpp FORM_*"""
         self.case = case
         self.p = make_params(case, recon)
+        self.p.form = {"difference": 0, "textbook": 1}[form]
         self.neq = 2 * case.nfluids + case.ndim + 1
         self.shape = (self.neq, case.n[2], case.n[1], case.n[0])
 

@@ -9,8 +9,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
-# MFC_B200_LIB names another library file to build/load (tuning variants); MFC_B200_NVCC_EXTRA adds nvcc flags.
-LIB = os.environ.get("MFC_B200_LIB") or os.path.join(HERE, "libmfc_b200.so")
+LIB = os.path.join(HERE, "libmfc_b200.so")
 SRC = [os.path.join(HERE, "csrc", "mfc_b200.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "mfc_device.cuh"), os.path.join(ROOT, "include", "mfc_b200.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -32,9 +31,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         fcntl.flock(lock, fcntl.LOCK_EX)
         try:
             if force or not _fresh():
-                extra = os.environ.get("MFC_B200_NVCC_EXTRA", "").split()
                 tmp = LIB + ".tmp.%d" % os.getpid()
-                cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC
+                cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SRC
                 subprocess.check_call(cmd)
                 os.replace(tmp, LIB)
         finally:

@@ -28,31 +28,15 @@ constexpr unsigned FULL = 0xffffffffu;
 // The template parameter WV of the sweeps encodes the nonlinear weights (WV % 3: WENO_JS / WENO_M / WENO_Z) and the
 // volume-fraction model (WV / 3: 0 Allaire, 1 Kapila) — both compile-time, so that neither costs the other anything.
 #define KAPILA_ON(kp) (WV >= 3)
-// Tuning knobs (compile-time; the defaults are the measured best on B200).
-#ifndef MFC_XW
-#define MFC_XW 4          // warps per block, sweep_x
-#endif
-#ifndef MFC_XMINB
-#define MFC_XMINB 3       // __launch_bounds__ min blocks per SM, sweep_x (168 registers: 12 warps per SM)
-#endif
-#ifndef MFC_MB
-#define MFC_MB 128        // threads per block, sweep_march
-#endif
-#ifndef MFC_MMINB
-#define MFC_MMINB 1       // __launch_bounds__ min blocks per SM, sweep_march
-#endif
-#ifndef MFC_MUNROLL
-#define MFC_MUNROLL 1    // unroll factor of the marching loop, sweep_march
-#endif
-constexpr int XW = MFC_XW;
-constexpr int MUNROLL = MFC_MUNROLL;
-constexpr int MB = MFC_MB;
+// Launch shapes (the measured best on B200).
+constexpr int XW = 4;      // warps per block, sweep_x
+constexpr int XMINB = 3;   // __launch_bounds__ min blocks per SM, sweep_x (168 registers: 12 warps per SM)
+constexpr int MB = 128;    // threads per block, sweep_march
 constexpr int PB = 256;   // threads per block, pointwise kernels
 
 // ------------------------------------------------------------------------------------------------ prim
 template <int N, int D>
-__global__ void __launch_bounds__(PB) prim_kernel(const __grid_constant__ KP kp, const double* __restrict__ q,
-                                                  double* __restrict__ w) {
+__global__ void __launch_bounds__(PB) prim_kernel(const __grid_constant__ KP kp, const double* q, double* w) {  // q, w may alias
   constexpr int NEQ = 2 * N + D + 1;
   const long long c = (long long)blockIdx.x * PB + threadIdx.x;
   if (c >= kp.ncells) return;
@@ -121,7 +105,7 @@ struct XCursor {
 };
 
 template <int N, int D, bool ACCUM, int STAGE, int WV>
-__global__ void __launch_bounds__(XW * 32, MFC_XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
+__global__ void __launch_bounds__(XW * 32, XMINB) sweep_x(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                    double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt,
                                                    int chunk, unsigned* next_chunk, unsigned* reset_other) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
@@ -290,18 +274,22 @@ __device__ __forceinline__ void cp_async8(double* sdst, const double* gsrc) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 constexpr int MARCH_RING = 8;  // 3 w + 3 d + 2 u slots
-__host__ __device__ constexpr int march_slots(bool accum, int stage) {
-  return MARCH_RING + (accum ? 1 : 0) + (stage >= 1 ? 1 : 0) + (stage >= 2 ? 1 : 0);
+// The cell of the stage state (RK stages 2, 3) is staged like the other operands of the update unless that slot would push
+// the block over half of the SM's shared memory (NEQ >= 9: 11 slots = 112 KB, one block per SM); then it is read directly
+// (it was loaded three steps earlier as cell g+2 of the sweep: an L1/L2 hit).  Config 5: z sweeps 10.7 -> 10.2 ms.
+__host__ __device__ constexpr bool march_qs_staged(int neq, int stage) { return stage >= 2 && neq <= 8; }
+__host__ __device__ constexpr int march_slots(bool accum, int stage, int neq) {
+  return MARCH_RING + (accum ? 1 : 0) + (stage >= 1 ? 1 : 0) + (march_qs_staged(neq, stage) ? 1 : 0);
 }
 
 template <int N, int D, int DIR, bool ACCUM, int STAGE, int WV>
-__global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
+__global__ void __launch_bounds__(MB, 1) sweep_march(const __grid_constant__ KP kp, const double* __restrict__ q,
                                                   double* __restrict__ rhs, int seglen, int nseg, double* qnn, double dt) {
   constexpr int NEQ = 2 * N + D + 1, IA = N + D + 1;
   constexpr int NH = (NEQ + 1) / 2;  // variables are stored in pairs (double2) so that every ring access moves two
   constexpr int SLOT = NH * MB;      // double2 per slot
   constexpr int S_D = 3, S_U = 6, S_ACC = MARCH_RING, S_QN = MARCH_RING + (ACCUM ? 1 : 0), S_QS = S_QN + 1;
-  extern __shared__ double2 ring[];  // PAIR: [slots][NH][MB] double2 = variables (2h, 2h+1); else [slots][2 NH][MB] doubles
+  extern __shared__ double2 ring[];  // [slots][NH][MB] double2 = variables (2h, 2h+1)
   const int n = kp.n[DIR];
   const int ncols = (int)(kp.ncells / n);
   const long long id = (long long)blockIdx.x * MB + threadIdx.x;
@@ -323,34 +311,14 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
   const int L = min(seglen, n - s0);
   const int lo = kp.bc_lo[DIR], hi = kp.bc_hi[DIR];
   const double idx = kp.inv_dx[DIR];
-#ifndef MFC_PAIR
-#define MFC_PAIR 1
-#endif
-  constexpr bool PAIR = MFC_PAIR != 0;
   // BF: the prefetch and the cp.async staging are issued unconditionally (on a valid, unused cell outside their range)
   // instead of under a branch.  Measured on B200: 2 % faster for z, 3.5 % slower for y.
-#ifndef MFC_BF
-#define MFC_BF (DIR == 2)
-#endif
-  constexpr bool BF = MFC_BF;
-  // element (double2 offset o within the ring, pair h): one 16-byte access (PAIR) or two 8-byte accesses
-  auto ld2 = [&](int o, int h) -> double2 {
-    if (PAIR) return ring[o + h * MB + threadIdx.x];
-    const double* b = reinterpret_cast<const double*>(ring) + 2 * o + 2 * h * MB + threadIdx.x;
-    return make_double2(b[0], b[MB]);
-  };
-  auto st2 = [&](int o, int h, double2 x) {
-    if (PAIR) {
-      ring[o + h * MB + threadIdx.x] = x;
-    } else {
-      double* b = reinterpret_cast<double*>(ring) + 2 * o + 2 * h * MB + threadIdx.x;
-      b[0] = x.x;
-      b[MB] = x.y;
-    }
-  };
+  constexpr bool BF = DIR == 2;
+  // element (double2 offset o within the ring, pair h): one 16-byte access
+  auto ld2 = [&](int o, int h) -> double2 { return ring[o + h * MB + threadIdx.x]; };
+  auto st2 = [&](int o, int h, double2 x) { ring[o + h * MB + threadIdx.x] = x; };
   auto elem = [&](int o, int v) -> double* {  // address of variable v in the slot at double2 offset o
-    double* b = reinterpret_cast<double*>(ring);
-    return PAIR ? b + 2 * (o + (v / 2) * MB + threadIdx.x) + (v & 1) : b + 2 * o + v * MB + threadIdx.x;
+    return reinterpret_cast<double*>(ring) + 2 * (o + (v / 2) * MB + threadIdx.x) + (v & 1);
   };
 #define RG(slot, v) (*elem((slot) * SLOT, (v)))
   bool bad = false;
@@ -419,7 +387,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
 #pragma unroll
   for (int v = 0; v < NEQ; ++v) WLp[v] = Fp[v] = 0.0;
   int offc = base + (s0 - 2) * stride;      // cell g-1 of step p (used for p >= 2)
-#pragma unroll(MUNROLL)
+#pragma unroll 1
   for (int p = 0; p <= L + 1; ++p) {
     double am[N];  // alpha_i of cell g-1 (source term of its update), read before its slot is reused
 #pragma unroll
@@ -446,7 +414,7 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
       for (int v = 0; v < NEQ; ++v) {
         if (ACCUM) cp_async8(&RG(S_ACC, v), rhs + v * kp.ncells + offs);
         if (STAGE >= 1) cp_async8(&RG(S_QN, v), qnn + v * kp.ncells + offs);
-        if (STAGE >= 2) cp_async8(&RG(S_QS, v), q + v * kp.ncells + offs);
+        if (march_qs_staged(NEQ, STAGE)) cp_async8(&RG(S_QS, v), q + v * kp.ncells + offs);
       }
       cp_async_commit();
     }
@@ -504,7 +472,13 @@ __global__ void __launch_bounds__(MB, MFC_MMINB) sweep_march(const __grid_consta
 #pragma unroll
         for (int h = 0; h < NH; ++h) {
           const double2 a = ld2(S_QN * SLOT, h);
-          const double2 b = STAGE >= 2 ? ld2(S_QS * SLOT, h) : make_double2(0.0, 0.0);
+          double2 b = make_double2(0.0, 0.0);
+          if (march_qs_staged(NEQ, STAGE)) {
+            b = ld2(S_QS * SLOT, h);
+          } else if (STAGE >= 2) {
+            b.x = __ldg(q + (2 * h) * kp.ncells + offc);
+            if (2 * h + 1 < NEQ) b.y = __ldg(q + (2 * h + 1) * kp.ncells + offc);
+          }
           qnc[2 * h] = a.x;
           qsc[2 * h] = b.x;
           if (2 * h + 1 < NEQ) {
@@ -763,7 +737,6 @@ struct mfc_grid {
   double* d_dt = nullptr;               // [0] dt of the step in flight, [1] elapsed time (mfc_advance)
   unsigned* d_xnext = nullptr;          // two work counters of sweep_x, used alternately (each launch zeroes the other)
   int xparity = 0;
-  int xchunk = 0;                       // items per chunk (0 = default)
   unsigned long long* h_red = nullptr;  // pinned: [0] smax bits, [1] flag
   int seg[3];
   long long launches = 0;
@@ -890,7 +863,7 @@ static cudaError_t launch_march(mfc_grid* g, const double* q, double* rhs, doubl
     const int nseg = (n + seglen - 1) / seglen;
     const long long threads = g->kp.ncells / n * nseg;
     const long long nb = (threads + MB - 1) / MB;
-    const size_t smem = sizeof(double2) * march_slots(ACCUM, STAGE) * ((NEQ + 1) / 2) * MB;
+    const size_t smem = sizeof(double2) * march_slots(ACCUM, STAGE, NEQ) * ((NEQ + 1) / 2) * MB;
     auto kern = sweep_march<N, D, DIR, ACCUM, STAGE, WV>;
     static bool attr_done[16] = {};
     if (!attr_done[g->device & 15]) {
@@ -928,7 +901,6 @@ static cudaError_t launch_x(mfc_grid* g, const double* q, double* rhs, double* q
   long long chunk = items / (nb * XW * 8);
   if (chunk < 1) chunk = 1;
   if (chunk > 16) chunk = 16;
-  if (g->xchunk > 0) chunk = g->xchunk;
   unsigned* cur = g->d_xnext + (g->xparity & 1);
   unsigned* other = g->d_xnext + ((g->xparity + 1) & 1);
   g->xparity ^= 1;
@@ -959,7 +931,7 @@ static cudaError_t launch_rhs(mfc_grid* g, const double* q, double* rhs, int mas
   else {
   const int all = (1 << D) - 1;
   cudaError_t e;
-  if ((mask & all) == all && g->kp.eta > 0.0) {
+  if (mask == 7 && g->kp.eta > 0.0) {  // the viscous rates belong to the whole RHS only (dir_mask == 7, as in mfc_rhs)
     if ((e = launch_viscous<N, D>(g, q, rhs)) != cudaSuccess) return e;
     if ((e = launch_x<N, D, WV, true, 0>(g, q, rhs, nullptr, 0.0)) != cudaSuccess) return e;
   } else if ((mask & all) == all) {
@@ -1046,15 +1018,6 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
   return cudaGetLastError();
 }
 
-#ifdef MFC_ONLY_23  // tuning builds: one instantiation only
-#define MFC_DISPATCH(g, EXPR)                                  \
-  [&]() -> cudaError_t {                                       \
-    switch ((g)->nf * 10 + (g)->ndim) {                        \
-      case 23: { constexpr int N = 2, D = 3; return EXPR; }    \
-    }                                                          \
-    return cudaErrorInvalidValue;                              \
-  }()
-#else
 #define MFC_DISPATCH(g, EXPR)                                  \
   [&]() -> cudaError_t {                                       \
     switch ((g)->nf * 10 + (g)->ndim) {                        \
@@ -1070,16 +1033,8 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
     }                                                          \
     return cudaErrorInvalidValue;                              \
   }()
-#endif
 
 // the same with the weights variant WV of the handle as a third compile-time constant
-#ifdef MFC_ONLY_23
-#define MFC_DISPATCH_W(g, EXPR)                                                   \
-  [&]() -> cudaError_t {                                                          \
-    constexpr int WV = WENO_JS;                                                   \
-    return (g)->weno == WENO_JS && !(g)->kp.kapila ? MFC_DISPATCH(g, EXPR) : cudaErrorInvalidValue;  \
-  }()
-#else
 #define MFC_DISPATCH_W1(g, K, EXPR)                                                          \
   switch ((g)->weno) {                                                                           \
     case WENO_JS: { constexpr int WV = WENO_JS + 3 * K; return MFC_DISPATCH(g, EXPR); }          \
@@ -1095,7 +1050,6 @@ static cudaError_t launch_cfl(mfc_grid* g, const double* q) {
     }                                                                                            \
     return cudaErrorInvalidValue;                                                                \
   }()
-#endif
 
 template <int N, int D, int WV>
 static cudaError_t launch_rk3_stage(mfc_grid* g, double* q, double dt, int stage, int parts) {
@@ -1199,7 +1153,6 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, p->device) == cudaSuccess) g->num_sms = prop.multiProcessorCount;
   default_segments(g);
-  if (const char* xc = std::getenv("MFC_XCHUNK")) g->xchunk = std::atoi(xc);  // tuning knob (benchmarks only)
 
   const size_t bytes = state_bytes(g);
   cudaError_t e;

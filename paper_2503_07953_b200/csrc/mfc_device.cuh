@@ -133,18 +133,9 @@ __device__ __forceinline__ bool prim_cell(const KP& kp, const double* q, double*
 // operands: as literals ptxas re-materialises each of them with two UMOVs per loop iteration, and every
 // instruction that is not FP64 costs the sweeps an issue slot.
 enum { W_C133, W_03, W_06, W_01, W_5_60, W_M2_60, W_02, W_M005, W_M02, W_005, W_M01, W_2_60, W_M5_60, W_COUNT };
-#ifdef MFC_WC_LIT
-__device__ __forceinline__ constexpr double wc_lit(int i) {
-  constexpr double t[W_COUNT] = {13.0 / 3.0, 0.3, 0.6, 0.1, 5.0 / 60.0, -2.0 / 60.0, 0.2, -0.05, -0.2, 0.05, -0.1,
-                                 2.0 / 60.0, -5.0 / 60.0};
-  return t[i];
-}
-#define WCV(i) wc_lit(i)
-#else
 __constant__ double WC[W_COUNT] = {13.0 / 3.0, 0.3, 0.6, 0.1, 5.0 / 60.0, -2.0 / 60.0, 0.2, -0.05, -0.2, 0.05, -0.1,
                                    2.0 / 60.0, -5.0 / 60.0};
 #define WCV(i) WC[i]
-#endif
 
 __device__ __forceinline__ double weno5_u(double t, double eps4) { return fma(WCV(W_C133) * t, t, eps4); }
 
