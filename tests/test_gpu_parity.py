@@ -1,6 +1,6 @@
 """Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element, on the same
 seeded inputs.  Bars (BASELINE.json north_star): relative 1e-12 in the max-norm per
-variable group for one RHS evaluation, 1e-9 for the state after 100 RK3 steps; bit-exact for
+variable (momentum components: per group, parity_norm.py) for one RHS evaluation, 1e-9 for the state after 100 RK3 steps; bit-exact for
 mfc_prim_from_cons, the RK stage/clamp arithmetic on identical inputs, and mfc_cfl_dt.
 All tests here need a B200 (pytest -m gpu)."""
 from dataclasses import replace
@@ -163,6 +163,33 @@ def test_rhs_host_entry_point_matches_device_entry_point(torch, mfc):
     assert np.array_equal(out, base)
 
 
+# ------------------------------------------------------------------ against the paper's text in its textbook form
+@pytest.mark.parametrize("index,n", [(2, None), (3, 128), (4, 48), (5, 40), ("rough23", (33, 18, 11)), ("rough33", (40, 9, 13))])
+def test_rhs_agrees_with_textbook_form_oracle(torch, mfc, index, n):
+    """The first oracle writes WENO5-JS and HLLC in the evaluation forms N2 / N3, the forms the kernels use
+    too.  This test makes the parity claim independent of that choice: the oracle's second instantiation types the same two
+    definitions as the paper prints them (f = sum omega_r f^(r); F = F_K + S_K (q*_K - q_K)).
+    Against its fp64 evaluation the GPU is as close as that evaluation's own rounding allows: per variable within
+    4 x |textbook64 - textbook80| (plus the bar times the variable's scale, which is what is left where the textbook
+    evaluation happens to round well)."""
+    if isinstance(index, int):
+        case = W.config(index, n=n)
+        q = W.initial_state(case)
+    else:
+        case = make_case(3, int(index[-2]), n, W.BC_PERIODIC)
+        q = rough_state(case, 8)
+    tb = O.Oracle(case, form="textbook")
+    t64, t80 = tb.rhs(q), tb.rhs_ld(q)
+    assert tb.bad == 0
+    got = gpu_rhs(torch, mfc, case, q)
+    noise = group_noise(t64, t80, case.nfluids, case.ndim)
+    # per variable: |gpu - textbook64| <= 4 |textbook64 - textbook80| + bar
+    for v in range(case.neq):
+        scale = np.abs(t64[v]).max() if not (case.nfluids <= v < case.nfluids + case.ndim) else \
+            np.abs(t64[case.nfluids:case.nfluids + case.ndim]).max()
+        assert np.abs(got[v] - t64[v]).max() <= 4.0 * noise[v] + RHS_TOL * max(scale, 1e-300), (v, noise[v])
+
+
 # ------------------------------------------------------------------ full-size parity (the bench launch configurations)
 def test_rhs_full_size_config4_elementwise(torch, mfc):
     case = W.config(4)  # 256^3, the configuration bench.py times; every cell, bare bar
@@ -230,6 +257,115 @@ def test_rhs_full_size_config5_sampled(torch, mfc):
     boxes += [tuple(int(v) for v in rng.integers(0, n - 16, 3)) for _ in range(6)]
     worst, per = _sampled_box_parity(torch, mfc, case, q, boxes, core=16)
     assert worst <= RHS_TOL, per
+
+
+# ------------------------------------------------------------------ full-size parity THROUGH THE FUSED-STAGE KERNELS
+# mfc_advance (what bench.py times) = CFL reduction + the STAGE = 1, 2, 3 instantiations of the sweeps, at the launch shape
+# of the full-size grids (64-cell y/z segments, one-wave x grid with the dynamic chunk counter).  PAPER.md:207-211 with 137-143.
+def _advance_vs_oracle(torch, mfc, case, nsteps=1):
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    ref = q.copy()
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    t_gpu = g.advance(qd, case.cfl, nsteps)
+    t_ref = 0.0
+    for _ in range(nsteps):
+        dt = orc.cfl_dt(ref, case.cfl)
+        orc.rk3_step(ref, dt)
+        assert orc.bad == 0
+        t_ref += dt
+    got = qd.cpu().numpy()
+    g.close()
+    assert t_gpu == t_ref  # the device-side time step is the oracle's, bit for bit
+    # the bar of a state after RK3 steps; the increment q^{n+1} - q^n is held to the one-RHS bar relative to its own size
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    inc_worst, inc_per = rel_err(got - q, ref - q, case.nfluids, case.ndim)
+    return worst, per, inc_worst, inc_per
+
+
+def test_advance_full_size_config4_elementwise(torch, mfc):
+    worst, per, inc_worst, inc_per = _advance_vs_oracle(torch, mfc, W.config(4))  # 256^3, every cell
+    assert worst <= 1e-12, per          # one step: far inside the 1e-9 bar of 100 steps
+    assert inc_worst <= 1e-10, inc_per  # q^{n+1} - q^n = dt * (combination of three L's), relative to its own maximum
+
+
+def test_advance_full_size_config3_elementwise(torch, mfc):
+    worst, per, inc_worst, inc_per = _advance_vs_oracle(torch, mfc, W.config(3), nsteps=2)  # 1024^2 in full
+    assert worst <= 1e-12, per
+    # the volume fractions do not change at t = 0 except at round-off level (the bubble is at rest ahead of the shock):
+    # their increment has no scale of its own, the other variables do
+    # (nor does the partial density of the light gas, a trace wherever the fluid moves): their increments have no scale of
+    # their own, the other variables' do
+    assert max(v for k, v in inc_per.items() if not k.startswith("alpha") and k != "arho2") <= 1e-10, inc_per
+
+
+def test_advance_full_size_config5_sampled(torch, mfc, capsys):
+    """One CFL + RK3 step of config 5 at the largest n the host holds (512 when there is memory for the 10.7 GB input),
+    compared on sampled 16^3 boxes: the oracle steps a sub-box cut out of q with a 9-cell rim (three stages of a 3-cell
+    stencil), with the time step of the full grid."""
+    import psutil
+    avail = psutil.virtual_memory().available
+    n = 512 if avail > 40e9 else 320
+    if avail > 40e9:
+        assert n == 512
+    case = W.config(5, n=n)
+    q = W.initial_state(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    dt = g.cfl_dt(qd, case.cfl)
+    g.rk3_step(qd, dt)
+    g.check()
+    rng = np.random.default_rng(3)
+    at = lambda x, y, z: (int(x * n), int(y * n), int(z * n))
+    core, rim = 16, 9
+    boxes = [at(0.2, 0.5, 0.5), at(0.19, 0.1, 0.9), at(0.3, 0.5, 0.5), at(0.45, 0.35, 0.5), at(0.58, 0.5, 0.5),
+             at(0.7, 0.2, 0.3), at(0.84, 0.7, 0.6), (0, 0, 0), (n - core, n - core, n - core), (0, n // 2, n - core)]
+    boxes += [tuple(int(v) for v in rng.integers(0, n - core, 3)) for _ in range(4)]
+    gots, refs, olds = [], [], []
+    for lo3 in boxes:
+        idx = [np.clip(np.arange(lo3[d] - rim, lo3[d] + core + rim), 0, n - 1) for d in range(3)]  # extrapolation ends
+        sub = np.ascontiguousarray(q[:, idx[2][:, None, None], idx[1][None, :, None], idx[0][None, None, :]])
+        nn = tuple(len(idx[d]) for d in range(3))
+        scase = W.Case("box", 3, nn, case.dx, case.nfluids, case.gamma, case.pi_inf, (W.BC_EXTRAP,) * 3, (W.BC_EXTRAP,) * 3,
+                       weno_eps=case.weno_eps, alpha_floor=case.alpha_floor, clamp=case.clamp)
+        cut = (slice(None), slice(rim, rim + core), slice(rim, rim + core), slice(rim, rim + core))
+        olds.append(sub[cut].reshape(case.neq, -1).copy())
+        orc = O.Oracle(scase)
+        orc.rk3_step(sub, dt)
+        assert orc.bad == 0
+        refs.append(sub[cut].reshape(case.neq, -1))
+        gi = [torch.as_tensor(idx[d][rim:rim + core], device="cuda") for d in range(3)]
+        got = qd.view(case.shape)[:, gi[2][:, None, None], gi[1][None, :, None], gi[0][None, None, :]]
+        gots.append(got.cpu().numpy().reshape(case.neq, -1))
+    g.close()
+    got, ref, old = np.concatenate(gots, 1), np.concatenate(refs, 1), np.concatenate(olds, 1)
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    with capsys.disabled():
+        print(f"\n[config 5 step parity] n = {n} ({avail / 1e9:.0f} GB of host memory available), {len(boxes)} boxes, worst e_v = {worst:.2e}")
+    assert worst <= 1e-12, per
+    assert not np.array_equal(got, old)  # the step did move the sampled cells
+
+
+@pytest.mark.parametrize("seg", [(64, 64, 64), (30, 8, 8), (1000, 1000, 1000), (62, 9, 11), (7, 3, 2)])
+def test_rk3_step_independent_of_segmentation(torch, mfc, seg):
+    # the fused-stage kernels (STAGE = 1, 2, 3) partition the same faces whatever the segment lengths: bit-equal states,
+    # including the 64-cell segments and the whole-line segments of the full-size grids
+    case = make_case(3, 2, (140, 70, 67), W.BC_PERIODIC)
+    q = rough_state(case, 9)
+    outs = []
+    for sg in (None, seg):
+        g = mfc.Grid.from_case(case)
+        if sg:
+            g.set_segments(*sg)
+        qd = torch.from_numpy(q).cuda()
+        dt = 0.4 * g.cfl_dt(qd, 0.5)
+        for _ in range(2):
+            g.rk3_step(qd, dt)
+        g.check()
+        outs.append(qd.cpu().numpy())
+        g.close()
+    assert np.array_equal(outs[0], outs[1])
 
 
 # ------------------------------------------------------------------ RK3: stage arithmetic, clamp, 100 steps
@@ -445,16 +581,18 @@ def test_hllc_faces_unit_entry_point(torch, mfc, ndim, nfluids):
         for i in range(n):
             Fr[i], ur[i], bad = orc.hllc_face(d, wL[i], wR[i])
             assert bad == 0
-        # the measure of DESIGN.md §7: max-norm per variable group (here over the sample of faces)
+        # the measure of DESIGN.md §7 (parity_norm): max-norm per variable over the sample of faces, momentum components per group
+        worst, per = rel_err(F.T, Fr.T, nfluids, ndim)
+        worst = max(worst, np.abs(uf - ur).max() / np.abs(ur).max())
+        assert worst <= 1e-12, (d, per)
+        # beyond the contract, face by face against the face's OWN largest flux of the group.  DESIGN.md §7 derives the bar:
+        # inside one face rho u^2 + p and the star correction S_K rho (chi ds + (chi - 1) u_K) cancel to a flux that can be
+        # 10^2 times smaller than either (|u| up to 5e3 m/s, p down to 1e4 Pa here), so a face's own relative error is up
+        # to 10^2 * 2^-52 * (a few operations) ~ 1e-13 .. 1e-12; the bar is 1e-11.
         groups = [slice(0, nfluids), slice(nfluids, nfluids + ndim), slice(nfluids + ndim, nfluids + ndim + 1),
                   slice(nfluids + ndim + 1, neq)]
-        worst = max(np.abs(F[:, sl] - Fr[:, sl]).max() / np.abs(Fr[:, sl]).max() for sl in groups)
-        worst = max(worst, np.abs(uf - ur).max() / np.abs(ur).max())
-        # and face by face against the face's own largest flux of the group, one decade looser (cancellation between
-        # rho u^2 + p and the star correction inside one face)
         per_face = max((np.abs(F[:, sl] - Fr[:, sl]).max(axis=1) / np.abs(Fr[:, sl]).max(axis=1)).max() for sl in groups)
         assert per_face <= 1e-11, (d, per_face)
-        assert worst <= 1e-12, (d, worst)
     g.close()
 
 
@@ -815,7 +953,10 @@ def test_taylor_green_vortex_viscous_steps(torch, mfc):
     ke0, t = ke(q), 0.0
     for _ in range(40):
         dt = orc.cfl_dt(ref, 0.5)
-        assert g.cfl_dt(qd, 0.5) == pytest.approx(dt, rel=1e-12)
+        # the two time steps are reductions over two DIFFERENT states (the GPU's and the oracle's, a few ulp apart after the first
+        # step); on one and the same state mfc_cfl_dt is bit-exact (test_cfl_dt_bit_exact).  The first step starts from equal states.
+        dt_gpu = g.cfl_dt(qd, 0.5)
+        assert dt_gpu == dt if t == 0.0 else dt_gpu == pytest.approx(dt, rel=1e-12)
         orc.rk3_step(ref, dt)
         g.rk3_step(qd, dt)
         t += dt
