@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """bench.py — grind time of the MFC hot path on B200 (BASELINE.json metric), one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4|5|3|2|1] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4|5|3|2|1] [--impl ours|reference] [--no-also]
+    python bench.py --probe-fp64        (the FP64 DFMA probe alone, with its clock record: profiles/fp64_probe.json)
 
 A "step" is one pass of the whole hot path over the whole grid: the CFL reduction (mfc_cfl_dt) followed by
 one SSP-RK3 step = 3 x (x/y/z sweeps: cons->prim, WENO5-JS, HLLC, flux divergence, alpha div(u) source)
@@ -11,6 +12,12 @@ cells x equations) in ns, RHS evaluations = 3 per step.
 Default workload: BASELINE.json configs[3] (3D periodic two-fluid mixing, 256^3, 8 equations — the shape of
 the paper's Table-1 benchmark case), seeded synthetic input (mfc_workloads).  The state arrays
 (1.07 GB each, 4 of them touched per step) are far larger than the 126 MB L2, so no L2 flush is needed.
+
+With no --config (config 4, N = 1) the line also carries, under "also", configs 5 (512^3, 10 equations, 5 steps) and 3
+(1024^2, 50 steps), each with its own roofline and clock record.  "roofline" names the dominant kernel and the roof that
+binds it (north_star: "the slower of the two"): the floor times of that launch for the FP64 ALUs (algorithmic flops / derived
+peak) and for HBM (compulsory bytes of the kernel / measured copy bandwidth) are both printed, `frac` is against the larger;
+`frac_whole_step` is the algorithmic flop rate of the whole step against the FP64 peak.
 
 N > 1 (torchrun): the path runs on one GPU (north_star); ranks are independent replicas ("replicas only",
 DESIGN.md §9) — no data-path collective; time is the max over ranks, value the whole-job aggregate.
@@ -43,8 +50,10 @@ ALG_FLOPS_PER_CELL_RHS_BY_WENO = {"js": ALG_FLOPS_PER_CELL_RHS,
                                   "z": {1: 547.0, 2: 797.0, 3: 1844.6, 4: 3128.9, 5: 3867.6}}
 # FP64 peak "derived from unit counts and clocks": 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz.
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
-# DFMA-chain microbenchmark on this pool's B200: 17.05e12 DFMA/s = 34.1 TFLOP/s (SM clock ~1.80 GHz under FP64 load)
-FP64_PEAK_TFLOPS_MEASURED = 34.1
+# The measured counterpart is taken live in every run by mfc_measure_fp64 (DFMA chains, all SMs); a capture with its clock
+# record is kept in profiles/fp64_probe.json (made by `python bench.py --probe-fp64`).
+# One replica size per configuration for BOTH oracle timings (cpu_baseline and --impl reference); None = the configuration itself
+ORACLE_REPLICA_N = {1: None, 2: None, 3: 512, 4: 128, 5: 96}
 
 
 def env_int(name, default):
@@ -130,8 +139,13 @@ def grind_ns(ms, steps, cells, neq, replicas=1):
 
 
 def sweep_alg_bytes_per_cell(kernel, neq, ndim):
-    """compulsory HBM bytes per cell of one sweep kernel in the three-sweep design:
-    x reads q and writes rhs; y and z read q, read rhs and write rhs."""
+    """compulsory HBM bytes per cell of one launch of a sweep kernel inside an RK3 step of the three-sweep design
+    (DESIGN.md §6, §8): the first sweep (x) reads q and writes the partial L; a middle sweep reads q and L and writes L; the
+    last sweep of a stage (y in 2-D, z in 3-D; x in 1-D) also applies the RK stage: it reads q, L and — in stages 2 and 3,
+    where q^n is not the swept state — q^n, and writes the new stage state: (24 + 32 + 32)/3 per equation on average."""
+    last = {1: "sweep_x", 2: "sweep_y", 3: "sweep_z"}[ndim]
+    if kernel == last:
+        return ((16 if ndim == 1 else 24) + 8 * 2.0 / 3.0) * neq
     return (16 if kernel == "sweep_x" else 24) * neq
 
 
@@ -142,7 +156,7 @@ def run_reference(args, rank):
         return
     import mfc_workloads as W
     from oracle import oracle as O
-    n_ref = {1: None, 2: None, 3: 256, 4: 64, 5: 56}[args.config]
+    n_ref = ORACLE_REPLICA_N[args.config]
     case = dataclasses.replace(W.config(args.config, n=n_ref), weno=args.weno, model=args.model, eta=args.eta)
     q = W.initial_state(case)
     orc = O.Oracle(case)
@@ -170,7 +184,7 @@ def run_reference(args, rank):
 def cpu_baseline(config_index, weno="js", model="allaire", eta=0.0, budget_s=20.0):
     import mfc_workloads as W
     from oracle import oracle as O
-    n_ref = {1: None, 2: None, 3: 512, 4: 128, 5: 96}[config_index]
+    n_ref = ORACLE_REPLICA_N[config_index]
     case = dataclasses.replace(W.config(config_index, n=n_ref), weno=weno, model=model, eta=eta)
     q = W.initial_state(case)
     orc = O.Oracle(case)
@@ -188,45 +202,35 @@ def cpu_baseline(config_index, weno="js", model="allaire", eta=0.0, budget_s=20.
                       f"replica of config {config_index} ({sec:.1f} s of host time)"}
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)  # BASELINE.json config 4: "50 RK3 steps"
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
-    ap.add_argument("--n", type=int, default=None, help="override cells per direction (tests only)")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--weno", default="js", choices=["js", "m", "z"],
-                    help="nonlinear weights: js = BASELINE.json's WENO5-JS (default), m = mapped (the paper's default), z = WENO-Z")
-    ap.add_argument("--model", default="allaire", choices=["allaire", "kapila"], help="volume-fraction equation (kapila: two fluids)")
-    ap.add_argument("--eta", type=float, default=0.0, help="uniform shear viscosity (0: inviscid, BASELINE.json)")
-    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
-                    help="N > 1: independent replicas (default, DESIGN.md §9) or one periodic domain of N stacked slabs "
-                         "exchanging 3-layer halos over NCCL (weak scaling: every rank owns one configuration-sized slab)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-    rank, local_rank, world = env_int("RANK", 0), env_int("LOCAL_RANK", 0), env_int("WORLD_SIZE", 1)
-    if args.warmup < 3 and args.impl == "ours":
-        args.warmup = 3  # timing rule: at least 3 warm-up steps
+def median(xs):
+    xs = sorted(xs)
+    return xs[len(xs) // 2] if len(xs) % 2 else 0.5 * (xs[len(xs) // 2 - 1] + xs[len(xs) // 2])
 
-    if args.impl == "reference":
-        run_reference(args, rank)
-        return 0
 
-    import numpy as np
+def probe_fp64(M, local_rank):
+    """live DFMA probe with the clock record of the probe itself"""
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    try:
+        best = (0.0, 0.0)
+        for _ in range(3):  # ~60 ms of FP64 load per call: three calls so that nvidia-smi (100 ms period) sees the load
+            r = M.measure_fp64(local_rank)
+            best = (max(best[0], r[0]), max(best[1], r[1]))
+    except Exception as exc:  # a library without the probe
+        sampler.stop()
+        return None, None, {"error": str(exc)}
+    return best[0], best[1], sampler.stop()
+
+
+def measure(args, config_index, steps, rank, local_rank, world, with_e2e):
+    """Times `steps` steps of one configuration (device-resident), the per-kernel profile and the roofline figures.
+    Returns the dict of that configuration (value, ms_per_step, clocks, roofline, ...)."""
     import torch
     import mfc_workloads as W
     import paper_2503_07953_b200 as M
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device — the hot path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    case = dataclasses.replace(W.config(args.config, n=args.n), weno=args.weno, model=args.model, eta=args.eta)
+    case = dataclasses.replace(W.config(config_index, n=args.n if config_index == args.config else None),
+                               weno=args.weno, model=args.model, eta=args.eta)
     q0 = W.initial_state(case)
     slab = None
     if args.decomp == "slab":
@@ -264,7 +268,7 @@ def main():
         barrier()
         sampler.start()
         ev0.record()
-        advance(qd, case.cfl, args.steps)
+        advance(qd, case.cfl, steps)
         ev1.record()
         torch.cuda.synchronize()
         clocks = sampler.stop()
@@ -275,66 +279,88 @@ def main():
         clocks["attempt"] = attempt
         if not (bad_reasons & set(clocks.get("reasons") or [])):
             break
-    value = grind_ns(ms, args.steps, cells, neq, world)
+    value = grind_ns(ms, steps, cells, neq, world)
 
-    # ---- mfc_rhs alone (SURVEY §8(d) metric (i)): x, y, z sweeps without the RK stage, rhs written to its own array
+    # ---- SURVEY 8(d) "median of >= 10 repetitions": (b) single steps, each bracketed by its own events
+    reps = []
+    for _ in range(10):
+        ev0.record()
+        advance(qd, case.cfl, 1)
+        ev1.record()
+        torch.cuda.synchronize()
+        reps.append(ev0.elapsed_time(ev1))
+    step_median_ms = reduce_max_ms(median(reps), world)
+
+    # ---- (a) mfc_rhs alone (SURVEY 8(d) metric (i)): x, y, z sweeps without the RK stage, rhs written to its own array
     rhs_only = None
     if slab is None:
         rd = torch.empty_like(qd)
         for _ in range(3):
             g.rhs(qd, rd)
-        n_rhs = max(3, min(3 * args.steps, 30))
         torch.cuda.synchronize()
-        ev0.record()
-        for _ in range(n_rhs):
+        rr = []
+        for _ in range(11):
+            ev0.record()
             g.rhs(qd, rd)
-        ev1.record()
-        torch.cuda.synchronize()
-        r_ms = reduce_max_ms(ev0.elapsed_time(ev1), world) / n_rhs
-        rhs_only = {"value": r_ms * 1e6 / (cells * neq), "unit": "ns/cell/eqn/rhs_eval", "ms_per_rhs": r_ms, "evals": n_rhs,
-                    "call": "mfc_rhs"}
+            ev1.record()
+            torch.cuda.synchronize()
+            rr.append(ev0.elapsed_time(ev1))
+        r_ms = reduce_max_ms(median(rr), world)
+        rhs_only = {"value": r_ms * 1e6 / (cells * neq), "unit": "ns/cell/eqn/rhs_eval", "ms_per_rhs": r_ms, "evals": len(rr),
+                    "statistic": "median", "call": "mfc_rhs"}
         del rd
 
     # ---- per-kernel device times (CUDA events around every launch, on the launching stream) for the roofline
     g.set_profiling(True)
-    advance(qd, case.cfl, args.steps)
+    advance(qd, case.cfl, steps)
     prof = g.get_profile()
     g.set_profiling(False)
     tot_ms = sum(v[0] for v in prof.values())
-    kern = {k: {"ms_per_launch": v[0] / v[1], "launches_per_step": v[1] / args.steps, "share_of_step": v[0] / tot_ms}
+    kern = {k: {"ms_per_launch": v[0] / v[1], "launches_per_step": v[1] / steps, "share_of_step": v[0] / tot_ms}
             for k, v in prof.items() if v[1]}
     sweeps = [k for k in ("sweep_x", "sweep_y", "sweep_z") if k in kern]
     dom = max(sweeps, key=lambda k: kern[k]["ms_per_launch"] * kern[k]["launches_per_step"])
     dur_s = kern[dom]["ms_per_launch"] * 1e-3
-    flops_launch = ALG_FLOPS_PER_CELL_RHS_BY_WENO[args.weno][args.config] / case.ndim * cells
+    flops_rhs = ALG_FLOPS_PER_CELL_RHS_BY_WENO[args.weno][config_index] * cells
+    flops_launch = flops_rhs / case.ndim
     bytes_launch = sweep_alg_bytes_per_cell(dom, neq, case.ndim) * cells
     hbm_peak, hbm_src = measured_peaks()
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu --set full capture
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(f"config{args.config}", {}).get(dom)
-    # live FP64 probe (register-resident DFMA chains, all SMs): the measured counterpart of the derived peak
-    try:
-        dfma_tf, dfma3_tf = M.measure_fp64(local_rank)
-    except Exception:  # an older library without the probe
-        dfma_tf, dfma3_tf = FP64_PEAK_TFLOPS_MEASURED, None
-    roofline = {
-        "kernel": dom, "bound": "alu", "achieved": flops_launch / dur_s / 1e12, "peak": FP64_PEAK_TFLOPS_DERIVED,
-        "unit": "TFLOP/s", "frac": flops_launch / dur_s / 1e12 / FP64_PEAK_TFLOPS_DERIVED, "traffic": traffic,
-        "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md §8); measured in this run by "
-                       "mfc_measure_fp64 (DFMA chains): see measured_dfma_tflops",
-        "measured_dfma_tflops": dfma_tf, "measured_dfma_three_register_operands_tflops": dfma3_tf,
-        "frac_of_measured_dfma_peak": flops_launch / dur_s / 1e12 / dfma_tf,
-        "alg_flops_per_launch": flops_launch, "alg_bytes_per_launch": bytes_launch, "ms_per_launch": dur_s * 1e3,
-        "hbm": {"achieved": bytes_launch / dur_s / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": bytes_launch / dur_s / 1e9 / hbm_peak,
-                "peak_source": hbm_src + " (MEASURED_PEAKS.json hbm_gbs)" if hbm_src == "measured" else "fallback of B200_PROFILING.md"},
-        "kernels": kern,
-    }
+            traffic = json.load(f).get(f"config{config_index}", {}).get(dom)
+    dfma_tf, dfma3_tf, probe_clocks = probe_fp64(M, local_rank)
+    alu = {"achieved": flops_launch / dur_s / 1e12, "peak": FP64_PEAK_TFLOPS_DERIVED, "unit": "TFLOP/s",
+           "frac": flops_launch / dur_s / 1e12 / FP64_PEAK_TFLOPS_DERIVED,
+           "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md §8)",
+           "measured_dfma_tflops": dfma_tf, "measured_dfma_three_register_operands_tflops": dfma3_tf,
+           "frac_of_measured_dfma_peak": (flops_launch / dur_s / 1e12 / dfma_tf) if dfma_tf else None,
+           "probe_clocks": probe_clocks, "alg_flops_per_launch": flops_launch}
+    hbm = {"achieved": bytes_launch / dur_s / 1e9, "peak": hbm_peak, "unit": "GB/s", "frac": bytes_launch / dur_s / 1e9 / hbm_peak,
+           "peak_source": hbm_src + " (MEASURED_PEAKS.json hbm_gbs)" if hbm_src == "measured" else "fallback of B200_PROFILING.md",
+           "alg_bytes_per_launch": bytes_launch,
+           "bytes_are": "compulsory bytes of this kernel in the three-sweep design (q, partial L, q^n read; new state written)"}
+    # north_star: "the roofline taken as the slower of the two": the roof with the larger floor time binds this launch
+    t_alu, t_hbm = flops_launch / (FP64_PEAK_TFLOPS_DERIVED * 1e12), bytes_launch / (hbm_peak * 1e9)
+    bound = "alu" if t_alu >= t_hbm else "hbm"
+    sel = alu if bound == "alu" else hbm
+    step_s = ms * 1e-3 / steps
+    # whole step: algorithmic flops of 3 RHS evaluations / algorithmic bytes of SURVEY 8(d) (RHS: 16 neq per cell; an RK stage
+    # re-reads q^n in stages 2, 3 and the CFL reduction reads q once: (3*16 + 2*8 + 8) neq per cell per step) over the step time
+    step_bytes = (3 * 16 + 2 * 8 + 8) * neq * cells
+    whole = {"alu_frac": 3 * flops_rhs / step_s / 1e12 / FP64_PEAK_TFLOPS_DERIVED, "alu_tflops": 3 * flops_rhs / step_s / 1e12,
+             "hbm_frac_algorithmic_bytes": step_bytes / step_s / 1e9 / hbm_peak, "alg_bytes_per_step": step_bytes,
+             "ms_per_step": step_s * 1e3}
+    roofline = {"kernel": dom, "bound": bound, "achieved": sel["achieved"], "peak": sel["peak"], "unit": sel["unit"],
+                "frac": sel["frac"], "traffic": traffic, "ms_per_launch": dur_s * 1e3,
+                "denominator": ("alu: derived FP64 peak 37.2 TFLOP/s" if bound == "alu" else "hbm: measured copy bandwidth") +
+                               "; floor times of this launch: alu %.3f ms, hbm %.3f ms" % (t_alu * 1e3, t_hbm * 1e3),
+                "alu": alu, "hbm": hbm, "frac_whole_step": whole["alu_frac"], "whole_step": whole, "kernels": kern}
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the state, the step, D2H of the state, every step
     e2e = None
-    if not args.no_e2e:
+    if with_e2e:
         qh = torch.from_numpy(q0.copy()).pin_memory()
         if slab is None:
             step_host = lambda: g.advance_host(qh, case.cfl, 1)  # syncs inside
@@ -348,7 +374,7 @@ def main():
             call = "pinned H2D copy + Slab.advance(q, cfl, 1) + D2H copy per step"
         for _ in range(2):
             step_host()
-        n_e2e = max(2, min(args.steps, 10))
+        n_e2e = max(2, min(steps, 10))
         barrier()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
@@ -359,25 +385,100 @@ def main():
                "d2h_bytes_per_step": 8 * neq * cells, "steps": n_e2e, "ms_per_step": e_ms / n_e2e,
                "call": call}
         del qh
-
-    out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms / args.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+    g.close()
+    del qd
+    torch.cuda.empty_cache()
+    return {
+        "value": value, "ms_per_step": ms / steps, "ms_per_step_median_of_10_single_steps": step_median_ms, "steps": steps,
         "config": {"workload": case.name, "grid": list(case.n[:case.ndim]), "cells": cells, "neq": neq, "nfluids": case.nfluids,
-                   "weno": {"js": "WENO5-JS", "m": "WENO5-M (mapped)", "z": "WENO5-Z"}[args.weno], "model": args.model, "eta": args.eta, "rhs_evals_per_step": 3, "parallelism": ("slabs along the last direction, %d x 3-layer halo exchanges per step" % (3 * 2) if slab is not None
+                   "weno": {"js": "WENO5-JS", "m": "WENO5-M (mapped)", "z": "WENO5-Z"}[args.weno], "model": args.model, "eta": args.eta,
+                   "rhs_evals_per_step": 3,
+                   "parallelism": ("slabs along the last direction, %d x 3-layer halo exchanges per step" % (3 * 2) if slab is not None
                                    else "replicas only" if world > 1 else "single GPU"),
                    "l2": "inputs larger than L2 (state array %.0f MB vs 126 MB L2)" % (8e-6 * neq * cells) if 8 * neq * cells > 3e8
                    else "working set fits L2: latency/L2-bound configuration, roofline target does not apply"},
-        "cell_updates_per_s": cells * world * args.steps / (ms * 1e-3),
+        "cell_updates_per_s": cells * world * steps / (ms * 1e-3),
         "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "rhs_only": rhs_only, "roofline": roofline,
-        "paper_context": "PAPER.md:720-726 Table 1 (other hardware, whole step): GH200 0.32, H100 SXM 0.38, A100 0.62 ns",
     }
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)  # BASELINE.json config 4: "50 RK3 steps"
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--n", type=int, default=None, help="override cells per direction (tests only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--weno", default="js", choices=["js", "m", "z"],
+                    help="nonlinear weights: js = BASELINE.json's WENO5-JS (default), m = mapped (the paper's default), z = WENO-Z")
+    ap.add_argument("--model", default="allaire", choices=["allaire", "kapila"], help="volume-fraction equation (kapila: two fluids)")
+    ap.add_argument("--eta", type=float, default=0.0, help="uniform shear viscosity (0: inviscid, BASELINE.json)")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default, DESIGN.md §9) or one periodic domain of N stacked slabs "
+                         "exchanging 3-layer halos over NCCL (weak scaling: every rank owns one configuration-sized slab)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="headline configuration only (default: config 4 plus, at N = 1, "
+                    "configs 5 and 3 under \"also\")")
+    ap.add_argument("--probe-fp64", action="store_true", help="only the FP64 DFMA probe with its clock record (profiles/fp64_probe.json)")
+    args = ap.parse_args()
+    rank, local_rank, world = env_int("RANK", 0), env_int("LOCAL_RANK", 0), env_int("WORLD_SIZE", 1)
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return 0
+
+    import torch
+    import paper_2503_07953_b200 as M
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if args.probe_fp64:
+        out = []
+        for _ in range(3):
+            dfma, dfma3, clocks = probe_fp64(M, local_rank)
+            out.append({"dfma_tflops": dfma, "dfma_three_register_operands_tflops": dfma3, "clocks_during_probe": clocks})
+        print(json.dumps({"command": "python bench.py --probe-fp64", "gpu": torch.cuda.get_device_name(local_rank),
+                          "derived_peak_tflops": FP64_PEAK_TFLOPS_DERIVED,
+                          "what": "mfc_measure_fp64: register-resident DFMA chains on all SMs, 8 chains per thread, 16 warps per SM; "
+                                  "x = fma(x, a, b) with loop-invariant a, b / fma of three distinct changing registers",
+                          "runs": out}, indent=1))
+        return 0
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    head = measure(args, args.config, args.steps, rank, local_rank, world, with_e2e=not args.no_e2e)
+    out = {
+        "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": head["ms_per_step"], "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+    }
+    for k in ("config", "cell_updates_per_s", "clocks", "gpu_launches", "e2e", "rhs_only", "roofline",
+              "ms_per_step_median_of_10_single_steps"):
+        out[k] = head[k]
+    out["paper_context"] = "PAPER.md:720-726 Table 1 (other hardware, whole step): GH200 0.32, H100 SXM 0.38, A100 0.62 ns"
+    # the other two configurations the target names ("the 3D configs") and the full-size 2-D one, each with its own roofline
+    # and clock record: config 5 (512^3, 10 equations, the largest single-GPU workload) and config 3 (1024^2)
+    if args.config == 4 and world == 1 and not args.no_also and args.n is None and args.decomp == "replicas":
+        also = {}
+        for idx, st in ((5, 5), (3, 50)):
+            try:
+                r = measure(args, idx, st, rank, local_rank, world, with_e2e=False)
+                also[r["config"]["workload"]] = {k: r[k] for k in (
+                    "value", "ms_per_step", "ms_per_step_median_of_10_single_steps", "steps", "config", "cell_updates_per_s",
+                    "clocks", "gpu_launches", "rhs_only", "roofline")}
+            except Exception as exc:  # e.g. not enough host or device memory for 512^3
+                also[str(idx)] = {"error": repr(exc)}
+        out["also"] = also
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.config, args.weno, args.model, args.eta)
     if rank == 0:
         print(json.dumps(out))
-    g.close()
     if world > 1:
         torch.distributed.destroy_process_group()
     return 0

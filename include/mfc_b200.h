@@ -93,7 +93,8 @@ typedef struct {
   int model;             /* mfc_model: 0 = MFC_MODEL_ALLAIRE; MFC_MODEL_KAPILA needs nfluids == 2 */
   double eta;            /* uniform shear viscosity of the viscous stress T = 2 eta (D - tr(D) I/3), PAPER.md:63-67 (eqs. 1-2),
                           * in the momentum and energy equations; second-order central differences at the faces (A22).
-                          * 0 = inviscid (BASELINE.json).  Not available with MFC_BC_HALO. */
+                          * 0 = inviscid (BASELINE.json).  With MFC_BC_HALO the stencil reads the velocities of the ghost
+                          * layer from the halo arrays. */
   int device;            /* CUDA device ordinal */
   void *stream;          /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = default */
 } mfc_params;
@@ -152,7 +153,8 @@ mfc_status mfc_rk3_stage(mfc_grid *g, double *q, double dt, int stage);
 /* The same stage in two parts, so that the halo exchange can run while the first part computes: parts = 1 launches the
  * sweeps of the directions before the last (they read no ghost layer of the last direction), parts = 2 the sweep of the
  * last direction with the RK combination and clamp (it needs the halos), parts = 3 both (== mfc_rk3_stage).  Call part 1
- * before part 2, on the same q and dt.  In 1-D part 1 is empty. */
+ * before part 2, on the same q and dt.  In 1-D part 1 is empty; with eta > 0 on a handle with MFC_BC_HALO too (the viscous
+ * stencil reads the ghost layer of the last direction), and part 2 is then the whole stage. */
 mfc_status mfc_rk3_stage_parts(mfc_grid *g, double *q, double dt, int stage, int parts);
 mfc_status mfc_stage_input(mfc_grid *g, const double *q, int stage, const double **state_out);
 

@@ -612,6 +612,27 @@ __global__ void __launch_bounds__(PB) velocity_kernel(const __grid_constant__ KP
   for (int d = 0; d < D; ++d) vel[d * kp.ncells + c] = __ddiv_rn(q[(N + d) * kp.ncells + c], rho);
 }
 
+// the same for the ghost layer next to each end of the last direction that takes its ghost cells from a halo array
+// (layer 2 of halo_lo = cell -1, layer 0 of halo_hi = cell n; halo layout [neq][3][plane])
+template <int N, int D>
+__global__ void __launch_bounds__(PB) velocity_halo_kernel(const __grid_constant__ KP kp, double* vel_lo, double* vel_hi) {
+  const long long plane = kp.ncells / kp.n[D - 1];
+  const long long c = (long long)blockIdx.x * PB + threadIdx.x;
+  if (c >= plane) return;
+#pragma unroll
+  for (int end = 0; end < 2; ++end) {
+    const double* h = end ? kp.halo_hi : kp.halo_lo;
+    double* out = end ? vel_hi : vel_lo;
+    if (!h || (end ? kp.bc_hi[D - 1] : kp.bc_lo[D - 1]) != BC_HALO) continue;
+    const int layer = end ? 0 : 2;
+    double rho = h[(0 * 3 + layer) * plane + c];
+#pragma unroll
+    for (int i = 1; i < N; ++i) rho = __dadd_rn(rho, h[(i * 3 + layer) * plane + c]);
+#pragma unroll
+    for (int d = 0; d < D; ++d) out[d * plane + c] = __ddiv_rn(h[((N + d) * 3 + layer) * plane + c], rho);
+  }
+}
+
 template <int N, int D>
 __global__ void __launch_bounds__(PB) viscous_kernel(const __grid_constant__ KP kp, const double* __restrict__ vel,
                                                      double* __restrict__ rhs) {
@@ -637,13 +658,26 @@ __global__ void __launch_bounds__(PB) viscous_kernel(const __grid_constant__ KP 
       nb[d][2] = d < D ? ghost_index(i + 1, n, kp.bc_lo[d], kp.bc_hi[d]) : 0;
     }
   }
-  int rowbase[3][3];  // (k', j') -> offset of the row, 32-bit (fewer than 2^31 cells)
+  // the three layers of the last direction: base of component 0 and the stride between components — the interior array, or
+  // (MFC_BC_HALO: a slab end) the ghost layer's velocities
+  constexpr int LD = D - 1;
+  const int plane = (int)(kp.ncells / kp.n[LD]);  // cells of one layer of the last direction
+  const double* lbase[3];
+  long long lstride[3];
 #pragma unroll
-  for (int oz = 0; oz < 3; ++oz)
+  for (int o = 0; o < 3; ++o) {
+    lbase[o] = vel + (long long)nb[LD][o] * plane;
+    lstride[o] = kp.ncells;
+  }
+  if (D >= 2 && ijk[LD] == 0 && kp.bc_lo[LD] == BC_HALO) lbase[0] = kp.vel_halo_lo, lstride[0] = plane;
+  if (D >= 2 && ijk[LD] == kp.n[LD] - 1 && kp.bc_hi[LD] == BC_HALO) lbase[2] = kp.vel_halo_hi, lstride[2] = plane;
+  int rowoff[3];  // D = 3: offset of row j' within a layer, 32-bit (fewer than 2^31 cells)
 #pragma unroll
-    for (int oy = 0; oy < 3; ++oy) rowbase[oz][oy] = (nb[2][oz] * ny + nb[1][oy]) * nx;
+  for (int oy = 0; oy < 3; ++oy) rowoff[oy] = D == 3 ? nb[1][oy] * nx : 0;
   auto U = [&](int m, const int* o) {  // velocity component m at offset o[3] from the cell
-    return __ldg(vel + m * kp.ncells + (rowbase[o[2] + 1][o[1] + 1] + nb[0][o[0] + 1]));
+    const int ol = o[LD] + 1;
+    const int inplane = D == 1 ? 0 : (D == 3 ? rowoff[o[1] + 1] : 0) + nb[0][o[0] + 1];
+    return __ldg(lbase[ol] + m * lstride[ol] + inplane);
   };
   double acc[D + 1];
 #pragma unroll
@@ -730,6 +764,7 @@ struct mfc_grid {
   double* q1 = nullptr;     // stage state
   double* Lq = nullptr;     // rhs scratch
   double* vel = nullptr;    // velocities u_d (D arrays), only when eta > 0
+  double* vel_halo = nullptr;  // with MFC_BC_HALO: velocities of the ghost layer next to each end, [2][D][plane]
   double* hq = nullptr;     // device staging for the *_host calls (lazy)
   double* hr = nullptr;
   unsigned long long* d_red = nullptr;  // [0] = smax bits
@@ -806,6 +841,13 @@ static void drain_profile(mfc_grid* g) {
     g->pool.push_back(r.b);
   }
   g->recs.clear();
+}
+
+// MFC_BC_HALO: which ends of the last direction take their ghost layers from the halo arrays
+static bool halo_lo_on(const mfc_grid* g) { return g->kp.bc_lo[g->ndim - 1] == BC_HALO; }
+static bool halo_hi_on(const mfc_grid* g) { return g->kp.bc_hi[g->ndim - 1] == BC_HALO; }
+static bool halo_missing(const mfc_grid* g) {
+  return (halo_lo_on(g) && !g->kp.halo_lo) || (halo_hi_on(g) && !g->kp.halo_hi);
 }
 
 static size_t state_bytes(const mfc_grid* g) { return sizeof(double) * (size_t)g->neq * (size_t)g->kp.ncells; }
@@ -919,6 +961,15 @@ static cudaError_t launch_viscous(mfc_grid* g, const double* q, double* rhs) {
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  if (g->vel_halo) {  // slab ends: the velocities of the ghost layer from the halo arrays
+    if constexpr (D >= 2) {
+      const long long plane = g->kp.ncells / g->kp.n[D - 1];
+      Scope sc(g, MFC_K_PRIM);
+      velocity_halo_kernel<N, D><<<(unsigned)((plane + PB - 1) / PB), PB, 0, g->stream>>>(
+          g->kp, g->vel_halo, g->vel_halo + (size_t)D * plane);
+      if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+  }
   Scope sc(g, MFC_K_PRIM);
   viscous_kernel<N, D><<<nb, PB, 0, g->stream>>>(g->kp, g->vel, rhs);
   return cudaGetLastError();
@@ -964,6 +1015,12 @@ static cudaError_t launch_stage(mfc_grid* g, const double* qs, double* work, dou
       if ((e = launch_viscous<N, D>(g, qs, work)) != cudaSuccess) return e;
     return visc ? launch_x<N, D, WV, true, STAGE>(g, qs, work, qn, dt) : launch_x<N, D, WV, false, STAGE>(g, qs, work, qn, dt);
   } else {
+    // on a slab the viscous stencil reads the ghost layer of the last direction: nothing of the stage can start before the halos
+    // have landed, so part 1 is empty and part 2 is the whole stage
+    if (visc && (halo_lo_on(g) || halo_hi_on(g))) {
+      if (!(parts & 2)) return cudaSuccess;
+      parts = 3;
+    }
     if (parts & 1) {
       if (visc)
         if ((e = launch_viscous<N, D>(g, qs, work)) != cudaSuccess) return e;
@@ -1061,12 +1118,6 @@ static cudaError_t launch_rk3_stage(mfc_grid* g, double* q, double dt, int stage
   }
 }
 
-// MFC_BC_HALO: which ends of the last direction take their ghost layers from the halo arrays
-static bool halo_lo_on(const mfc_grid* g) { return g->kp.bc_lo[g->ndim - 1] == BC_HALO; }
-static bool halo_hi_on(const mfc_grid* g) { return g->kp.bc_hi[g->ndim - 1] == BC_HALO; }
-static bool halo_missing(const mfc_grid* g) {
-  return (halo_lo_on(g) && !g->kp.halo_lo) || (halo_hi_on(g) && !g->kp.halo_hi);
-}
 
 static mfc_status use_device(const mfc_grid* g) {
   CK(cudaSetDevice(g->device));
@@ -1108,10 +1159,6 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
   if (p->model == MFC_MODEL_KAPILA && p->nfluids != 2)
     return fail(MFC_ERR_ARG, "mfc_init_grid: MFC_MODEL_KAPILA is defined for two fluids (PAPER.md:78, eq. 5)");
   if (!(p->eta >= 0.0)) return fail(MFC_ERR_ARG, "mfc_init_grid: eta must be >= 0");
-  if (p->eta > 0.0)
-    for (int d = 0; d < p->ndim; ++d)
-      if (p->bc_lo[d] == MFC_BC_HALO || p->bc_hi[d] == MFC_BC_HALO)
-        return fail(MFC_ERR_ARG, "mfc_init_grid: viscous terms are not available with MFC_BC_HALO");
   if (p->weno != MFC_WENO_JS && p->weno != MFC_WENO_M && p->weno != MFC_WENO_Z)
     return fail(MFC_ERR_ARG, "mfc_init_grid: weno must be MFC_WENO_JS, MFC_WENO_M or MFC_WENO_Z");
   int ndev = 0;
@@ -1171,6 +1218,16 @@ mfc_status mfc_init_grid(const mfc_params* p, mfc_grid** out) {
     mfc_free_grid(g);
     return fail(MFC_ERR_ALLOC, "mfc_init_grid: allocation of the velocity arrays failed");
   }
+  if (g->kp.eta > 0.0 && (halo_lo_on(g) || halo_hi_on(g))) {
+    const size_t plane = (size_t)(cells / p->n[p->ndim - 1]);
+    if (cudaMalloc(&g->vel_halo, sizeof(double) * 2 * (size_t)g->ndim * plane) != cudaSuccess) {
+      cudaGetLastError();
+      mfc_free_grid(g);
+      return fail(MFC_ERR_ALLOC, "mfc_init_grid: allocation of the halo velocities failed");
+    }
+    g->kp.vel_halo_lo = g->vel_halo;
+    g->kp.vel_halo_hi = g->vel_halo + (size_t)g->ndim * plane;
+  }
   g->kp.flag = g->d_flag;
   CK(cudaMemsetAsync(g->d_flag, 0, sizeof(int), g->stream));
   CK(cudaMemsetAsync(g->d_red, 0, 16, g->stream));
@@ -1186,6 +1243,7 @@ mfc_status mfc_free_grid(mfc_grid* g) {
   cudaFree(g->q1);
   cudaFree(g->Lq);
   cudaFree(g->vel);
+  cudaFree(g->vel_halo);
   cudaFree(g->hq);
   cudaFree(g->hr);
   cudaFree(g->d_red);

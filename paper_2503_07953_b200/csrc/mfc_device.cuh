@@ -29,6 +29,9 @@ struct KP {
   // BC_HALO on the last direction (slab decomposition): the three ghost layers beyond each end, [neq][3][plane]
   const double* halo_lo;
   const double* halo_hi;
+  // velocities of the ghost layer next to each such end, [D][plane] (viscous terms on a slab)
+  const double* vel_halo_lo;
+  const double* vel_halo_hi;
 };
 
 // O1: logical cell g in [-3, n+2] -> interior cell that supplies its value.

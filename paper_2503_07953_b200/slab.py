@@ -88,7 +88,9 @@ class Slab:
         self.case, self.start, self.count = local_case(case, rank, world)
         d = case.ndim - 1
         self.below, self.above = neighbours(rank, world, case.bc_lo[d] == BC_PERIODIC)
-        self.grid = Grid.from_case(self.case, device=device)
+        # the stream the kernels of the handle run on (Grid takes torch's current stream of the device at construction)
+        self.stream = torch.cuda.current_stream(device)
+        self.grid = Grid.from_case(self.case, device=device, stream=self.stream.cuda_stream)
         plane = self.case.cells // self.case.n[d]
         n = self.case.neq * 3 * plane
         mk = lambda: torch.empty(n, dtype=torch.float64, device=f"cuda:{device}")
@@ -111,10 +113,20 @@ class Slab:
         import torch
         self.pack(q, stage)
         if not (self.below == self.rank and self.above == self.rank):
-            torch.cuda.current_stream().synchronize()  # the packed buffers must be complete before NCCL reads them on its stream
+            # the packed buffers must be complete before NCCL reads them: NCCL's stream waits for the CURRENT stream when the
+            # transfers are posted, so the current stream is made to wait for an event recorded behind the packing — the
+            # host is not stalled (no synchronize; three per step in round 1)
+            cur = torch.cuda.current_stream(self.stream.device)
+            if cur != self.stream:
+                ev = torch.cuda.Event()
+                ev.record(self.stream)
+                cur.wait_event(ev)
         works = exchange(self.send_lo, self.send_hi, self.halo_lo, self.halo_hi, self.rank, self.below, self.above,
-                         self.dist, self.group, wait)
+                         self.dist, self.group, wait=False)
         self.exchanges += 1
+        if wait:
+            self._wait(works)
+            return []
         return works
 
     def rhs(self, q, out):
@@ -127,9 +139,21 @@ class Slab:
         for stage in (1, 2, 3):
             works = self.refresh(q, stage, wait=False)
             self.grid.rk3_stage(q, dt, stage, parts=1)
-            for w in works:
-                w.wait()
+            self._wait(works)
             self.grid.rk3_stage(q, dt, stage, parts=2)
+
+    def _wait(self, works):
+        """NCCL work.wait() makes the current stream wait for the transfer (no host stall); the handle's stream follows it"""
+        if not works:
+            return
+        import torch
+        for w in works:
+            w.wait()
+        cur = torch.cuda.current_stream(self.stream.device)
+        if cur != self.stream:
+            ev = torch.cuda.Event()
+            ev.record(cur)
+            self.stream.wait_event(ev)
 
     def cfl_dt(self, q, cfl):
         """global dt: the minimum over slabs of the local one (one scalar all-reduce)"""

@@ -81,7 +81,10 @@ def test_grind_time_arithmetic():
     assert bench.grind_ns(24.0, 10, 10 ** 6, 8) == pytest.approx(0.1)
     assert bench.grind_ns(24.0, 10, 10 ** 6, 8, replicas=2) == pytest.approx(0.05)
     assert bench.sweep_alg_bytes_per_cell("sweep_x", 8, 3) == 128
-    assert bench.sweep_alg_bytes_per_cell("sweep_z", 8, 3) == 192
+    assert bench.sweep_alg_bytes_per_cell("sweep_y", 8, 3) == 192           # middle sweep: q and L read, L written
+    assert bench.sweep_alg_bytes_per_cell("sweep_z", 8, 3) == pytest.approx(8 * (24 + 32 + 32) / 3)  # last sweep + RK stage, mean of 3
+    assert bench.sweep_alg_bytes_per_cell("sweep_y", 7, 2) == pytest.approx(7 * (24 + 32 + 32) / 3)
+    assert bench.median([3.0, 1.0, 2.0]) == 2.0 and bench.median([4.0, 1.0, 2.0, 3.0]) == 2.5
     assert bench.FP64_PEAK_TFLOPS_DERIVED == pytest.approx(37.225, rel=1e-3)
 
 
