@@ -139,3 +139,33 @@ def test_mixture_sound_speed_is_the_isentropic_derivative_of_the_eos(alpha_w):
     ci2 = [case.gamma[i] * (p0 + case.pi_inf[i]) / (arho[i] / a[i]) for i in range(2)]
     wood = 1.0 / (rho * sum(a[i] / ((arho[i] / a[i]) * ci2[i]) for i in range(2)))
     assert c_oracle ** 2 >= wood * (1 - 1e-12)
+
+
+# ------------------------------------------------------------------ what the CFL number of cfl_dt means (reading A9)
+def test_cfl_dt_scales_the_step_to_the_stability_limit_of_the_fastest_wave():
+    """A9 defines dt = CFL / max sum_d (|u_d| + c)/dx_d; nothing in the paper does.  What can be pinned is its meaning: with
+    first-order upwinding (piecewise-constant reconstruction + HLLC) each characteristic field of the linearised 1-D Euler
+    equations obeys dw/dt = -lambda (w_i - w_{i-1})/dx, and SSP-RK3 is stable for lambda dt/dx <= 1.2564 (|R(z)| <= 1 on
+    z = -nu (1 - exp(-i theta)) up to nu = 1.2564).  The fastest field has lambda = |u| + c, so a small perturbation of a
+    uniform state must stay bounded for CFL = 1.15 and blow up for CFL = 1.40.  A cfl_dt that used c alone, |u| alone, or
+    half / twice the spacing would fail one of the two."""
+    n = 64
+    case = advection_case(n)
+    rng = np.random.default_rng(5)
+    one = np.ones(case.shape[1:])
+    pert = lambda: 1e-7 * rng.standard_normal(case.shape[1:])
+    q0 = np.ascontiguousarray(W.cons_from_prim(case, [1.0 + pert()], [0.8 + pert()], 1.0 + pert(), [one]))  # u = 0.8, c = 1.18
+    orc = O.Oracle(case, recon=O.RECON_PC)
+    base = np.ascontiguousarray(W.cons_from_prim(case, [one], [0.8 * one], 1.0, [one]))
+
+    def growth(cfl, nsteps=400):
+        q = q0.copy()
+        dt = orc.cfl_dt(q, cfl)
+        assert dt == pytest.approx(cfl * (1.0 / n) / (0.8 + np.sqrt(1.4)), rel=1e-6)
+        for _ in range(nsteps):
+            orc.rk3_step(q, dt)
+        return np.abs(q - base).max() / np.abs(q0 - base).max()
+
+    assert growth(1.15) < 2.0
+    g = growth(1.40)
+    assert not (g < 1e3)  # grown beyond 10^3, or overflowed to inf / nan
