@@ -132,8 +132,8 @@ __device__ __forceinline__ bool prim_cell(const KP& kp, const double* q, double*
 // pieces (first differences d_k and u_k = 13/3 t_k^2 + 4 eps of the second differences t_k) from step to step
 // instead of recomputing them: weno5_u forms one u_k, weno5_core takes (c; d1..d4; u0..u2).
 // The coefficients live in constant memory so that they reach the FP64 instructions as constant-bank
-// operands: as literals ptxas re-materialises each of them with two UMOVs per loop iteration, and every
-// instruction that is not FP64 costs the sweeps an issue slot.
+// operands: as literals ptxas re-materialises each of them with two UMOVs per loop iteration (measured in round 1:
+// slower), instructions the loop does not need.
 enum { W_C133, W_03, W_06, W_01, W_5_60, W_M2_60, W_02, W_M005, W_M02, W_005, W_M01, W_2_60, W_M5_60, W_COUNT };
 __constant__ double WC[W_COUNT] = {13.0 / 3.0, 0.3, 0.6, 0.1, 5.0 / 60.0, -2.0 / 60.0, 0.2, -0.05, -0.2, 0.05, -0.1,
                                    2.0 / 60.0, -5.0 / 60.0};
