@@ -163,6 +163,42 @@ mfc_status mfc_stage_input(mfc_grid *g, const double *q, int stage, const double
  * q: device; dt_out: HOST pointer to one double.  syncs; also reports the sticky non-physical flag. */
 mfc_status mfc_cfl_dt(mfc_grid *g, const double *q, double cfl, double *dt_out);
 
+/* The same CFL time step for callers that must not allocate: no handle, no cudaMalloc / cudaFree /
+ * cudaMallocHost, nothing that grows the CUDA heap.  Meant for code that runs where device memory is
+ * not ours to take: a solver plugged into an application whose memory pool already owns all of HBM
+ * (another cudaMalloc fails or fragments the pool), a step function called from inside a latency-critical
+ * loop where an allocation is an implicit device-wide synchronisation, or a host that forbids allocation
+ * after start-up.  Every other call in this header needs an mfc_grid, and mfc_init_grid allocates.
+ *
+ * Only ndim, n, dx, nfluids, gamma, pi_inf, device and stream of *p are read (validated as in
+ * mfc_init_grid); the other fields are ignored.
+ *   q              device, neq*cells doubles, conservative state in the layout above (input, untouched)
+ *   cfl            CFL number
+ *   dt_out         DEVICE pointer to one double: receives cfl / max_cells sum_d (|u_d| + c)/dx_d, the same
+ *                  IEEE operations as mfc_cfl_dt, so the two agree bit for bit
+ *   nonphysical_out DEVICE pointer to one int, may be NULL: receives 1 if some cell had rho <= 0 or
+ *                  c^2 <= 0 or NaN (A19), else 0 — there is no handle to keep a sticky flag in
+ * async on p->stream; it never synchronises, which is why both results stay on the device.
+ *
+ * SCRATCH: the per-block partial maxima and the completion counter live in one array that is part of the
+ * library image, MFC_STATIC_SCRATCH_BYTES (129 KiB) on every GPU that loads the library, held until the
+ * process exits.  A block reduces MFC_STATIC_CELLS_PER_BLOCK cells and there is room for
+ * MFC_STATIC_MAX_BLOCKS partial results, so grids of more than MFC_STATIC_MAX_CELLS = 2^25 cells
+ * (256^3 fits, 512^3 does not) are refused with MFC_ERR_ARG and a text saying so; nothing is launched.
+ * The array is shared by every call in the process and keeps what the last call left there.  The call
+ * clears the counter and flag words it depends on before launching, so a call that follows an aborted
+ * one still starts clean — but two calls whose kernels overlap on one GPU (different streams, or
+ * different host threads) race on it and may both return garbage.  Serialise them.
+ *
+ * FIRST CALL on each device looks up the device address of that array (one cudaGetSymbolAddress with the
+ * device current, cached per device afterwards).  The lookup is not a stream operation, so make the
+ * first call on a device outside of any stream capture. */
+#define MFC_STATIC_CELLS_PER_BLOCK 2048
+#define MFC_STATIC_MAX_BLOCKS 16384
+#define MFC_STATIC_MAX_CELLS (1LL * MFC_STATIC_CELLS_PER_BLOCK * MFC_STATIC_MAX_BLOCKS)
+#define MFC_STATIC_SCRATCH_BYTES (8 * MFC_STATIC_MAX_BLOCKS + 1024)
+mfc_status mfc_cfl_dt_static(const mfc_params *p, const double *q, double cfl, double *dt_out, int *nonphysical_out);
+
 /* Syncs and returns MFC_ERR_NONPHYSICAL if any kernel since the last mfc_check flagged a non-physical
  * state (clears the flag), MFC_ERR_CUDA on an asynchronous CUDA error, else MFC_OK. */
 mfc_status mfc_check(mfc_grid *g);

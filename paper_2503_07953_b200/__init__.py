@@ -20,7 +20,8 @@ EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "m
            "mfc_rhs_dirs", "mfc_rk3_step", "mfc_rk3_steps", "mfc_cfl_dt", "mfc_check", "mfc_rhs_host",
            "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
            "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error", "mfc_set_halo", "mfc_rk3_stage",
-           "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64", "mfc_rk3_stage_parts")
+           "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64", "mfc_rk3_stage_parts", "mfc_cfl_dt_static")
+STATIC_MAX_CELLS = 2048 * 16384  # MFC_STATIC_MAX_CELLS of include/mfc_b200.h
 
 
 KERNEL_CLASSES = ("prim", "sweep_x", "sweep_y", "sweep_z", "rk", "cfl")
@@ -84,6 +85,7 @@ def lib():
         L.mfc_stage_input.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_void_p)]
         L.mfc_pack_halo.argtypes = [vp, dp, C.c_int, dp, dp]
         L.mfc_measure_fp64.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.mfc_cfl_dt_static.argtypes = [C.POINTER(MfcParams), dp, C.c_double, dp, dp]
         _lib = L
     return _lib
 
@@ -93,6 +95,37 @@ def measure_fp64(device=0):
     a, b = C.c_double(), C.c_double()
     _ck(lib().mfc_measure_fp64(int(device), None, C.byref(a), C.byref(b)))
     return a.value, b.value
+
+
+def cfl_dt_static(ndim, n, dx, gamma, pi_inf, q, cfl, dt_out, nonphysical_out=None, device=0, stream=None):
+    """mfc_cfl_dt_static: the CFL time step of state q without a Grid and without any allocation by the library.
+
+    For callers that cannot let the library allocate — a solver embedded in an application whose memory pool already
+    holds all of the GPU's memory, or a step loop in which an allocation would stall the device.  The reduction's
+    scratch is an array built into the library (129 KiB per GPU), which is why grids above STATIC_MAX_CELLS (2^25)
+    cells are refused, and why two calls that overlap on one GPU must be serialised by the caller (same stream).
+    q: CUDA float64 tensor, neq*cells elements; dt_out: CUDA float64 tensor of one element that receives dt;
+    nonphysical_out: CUDA int32 tensor of one element (or None) that receives 1 if a cell was non-physical, else 0.
+    Asynchronous on `stream` (default: torch's current stream); nothing is read back to the host here.  The first
+    call on a device looks up the array's device address: make it outside of stream capture."""
+    import torch
+    nf = len(gamma)
+    p = MfcParams()
+    p.ndim, p.nfluids, p.device = int(ndim), nf, int(device)
+    g_arr, pi_arr = (C.c_double * nf)(*gamma), (C.c_double * nf)(*pi_inf)
+    for d in range(3):
+        p.n[d] = n[d]
+        p.dx[d] = dx[d]
+    p.gamma = C.cast(g_arr, C.POINTER(C.c_double))
+    p.pi_inf = C.cast(pi_arr, C.POINTER(C.c_double))
+    p.stream = torch.cuda.current_stream(device).cuda_stream if stream is None else stream
+    count = (2 * nf + int(ndim) + 1) * int(n[0]) * int(n[1]) * int(n[2])
+    flag_ptr = None
+    if nonphysical_out is not None:
+        if not (nonphysical_out.is_cuda and nonphysical_out.dtype == torch.int32 and nonphysical_out.numel() == 1):
+            raise TypeError("nonphysical_out: expected a CUDA int32 tensor of one element")
+        flag_ptr = nonphysical_out.data_ptr()
+    _ck(lib().mfc_cfl_dt_static(C.byref(p), _dev_ptr(q, count), float(cfl), _dev_ptr(dt_out, 1), flag_ptr))
 
 
 def _ck(status):

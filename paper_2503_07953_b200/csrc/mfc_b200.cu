@@ -16,6 +16,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1554,3 +1555,181 @@ mfc_status mfc_get_profile(mfc_grid* g, int kernel_class, double* total_ms_host,
 }
 
 }  // extern "C"
+
+// ================================================================================================ mfc_cfl_dt_static
+// The CFL reduction for callers that cannot allocate (include/mfc_b200.h: an application whose memory pool owns all of
+// HBM, a latency-critical loop, a host that forbids allocation after start-up).  Everything the kernel needs beyond
+// its inputs and outputs — one partial maximum per block, the completion counter, the non-physical flag — sits in the
+// file-scope array below, which is part of the library image: MFC_STATIC_SCRATCH_BYTES on every GPU that loads the
+// library, until the process exits.  No handle, no cudaMalloc / cudaFree / cudaMallocHost on this path.
+//
+// `static_scratch` as written in HOST code is only the host-side shadow of the device array; handing that to a kernel
+// or to cudaMemsetAsync would fault (or, where the GPU can reach host memory, scribble over the shadow).  The host
+// therefore asks the runtime for the device address once per device (static_scratch_on) and passes that pointer.
+namespace mfc {
+
+constexpr int ST_CPB = MFC_STATIC_CELLS_PER_BLOCK;   // cells reduced by one block
+constexpr int ST_MAXB = MFC_STATIC_MAX_BLOCKS;       // partial maxima the array has room for
+constexpr int ST_HDR = 1024;                         // bytes in front of the partials: word 0 = blocks finished, word 1 = flag
+static_assert(ST_CPB % PB == 0, "a block's cells are dealt to its threads in whole rounds");
+static_assert(MFC_STATIC_SCRATCH_BYTES == ST_HDR + 8 * ST_MAXB, "header + one double per block");
+static __device__ __align__(256) unsigned char static_scratch[MFC_STATIC_SCRATCH_BYTES];
+
+// Same per-cell arithmetic as cfl_kernel (O7 / A9, every operation IEEE-rounded in the order of the definition), so the
+// maximum — which does not depend on the order of comparison — has the same bits.  What differs is where the partial
+// results go: block b stores its maximum in part[b]; the block that finishes last (counter in hdr[0]) takes the maximum
+// of the gridDim.x partials, writes dt and the flag to the caller's outputs and puts the counter and flag back to zero.
+template <int N, int D>
+__global__ void __launch_bounds__(PB) cfl_static_kernel(const __grid_constant__ KP kp, const double* __restrict__ q,
+                                                        double cfl, unsigned char* scratch, double* dt_out,
+                                                        int* nonphysical_out) {
+  constexpr int NEQ = 2 * N + D + 1, IM = N, IE = N + D, IA = N + D + 1;
+  unsigned* hdr = reinterpret_cast<unsigned*>(scratch);
+  double* part = reinterpret_cast<double*>(scratch + ST_HDR);
+  double smax = 0.0;
+  bool bad = false;
+  const long long c0 = (long long)blockIdx.x * ST_CPB + threadIdx.x;
+#pragma unroll 2
+  for (int k = 0; k < ST_CPB / PB; ++k) {
+    const long long c = c0 + (long long)k * PB;
+    if (c >= kp.ncells) break;
+    double qc[NEQ], w[NEQ];
+#pragma unroll
+    for (int v = 0; v < NEQ; ++v) qc[v] = q[v * kp.ncells + c];
+    bad |= prim_cell<N, D, true>(kp, qc, w);
+    double rho = w[0], Gam = __dmul_rn(w[IA], kp.G[0]), Pi = __dmul_rn(w[IA], kp.P[0]);
+#pragma unroll
+    for (int i = 1; i < N; ++i) {
+      rho = __dadd_rn(rho, w[i]);
+      Gam = __dadd_rn(Gam, __dmul_rn(w[IA + i], kp.G[i]));
+      Pi = __dadd_rn(Pi, __dmul_rn(w[IA + i], kp.P[i]));
+    }
+    const double c2 = __ddiv_rn(__dadd_rn(__dmul_rn(__dadd_rn(Gam, 1.0), w[IE]), Pi), __dmul_rn(Gam, rho));
+    bad |= !(c2 > 0.0);
+    const double cs = __dsqrt_rn(c2);
+    double s = __ddiv_rn(__dadd_rn(fabs(w[IM]), cs), kp.dx[0]);
+#pragma unroll
+    for (int d = 1; d < D; ++d) s = __dadd_rn(s, __ddiv_rn(__dadd_rn(fabs(w[IM + d]), cs), kp.dx[d]));
+    smax = s > smax ? s : smax;
+  }
+  __shared__ double wmax[PB / 32];
+  __shared__ bool last;
+  auto block_max = [&](double x) {  // maximum over the block, valid in thread 0
+#pragma unroll
+    for (int o = 16; o; o >>= 1) {
+      const double t = __shfl_xor_sync(FULL, x, o);
+      x = t > x ? t : x;
+    }
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = x;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+      x = threadIdx.x < PB / 32 ? wmax[threadIdx.x] : 0.0;
+#pragma unroll
+      for (int o = 16; o; o >>= 1) {
+        const double t = __shfl_xor_sync(FULL, x, o);
+        x = t > x ? t : x;
+      }
+    }
+    return x;
+  };
+  smax = block_max(smax);
+  const int any_bad = __syncthreads_or(bad ? 1 : 0);
+  if (threadIdx.x == 0) {
+    part[blockIdx.x] = smax;
+    if (any_bad) atomicOr(&hdr[1], 1u);
+    __threadfence();  // the partial and the flag are visible before the counter moves
+    last = atomicAdd(&hdr[0], 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  double m = 0.0;
+  for (unsigned b = threadIdx.x; b < gridDim.x; b += PB) {
+    const double t = __ldcg(part + b);  // written by other SMs: read it where they left it, in L2
+    m = t > m ? t : m;
+  }
+  m = block_max(m);
+  if (threadIdx.x == 0) {
+    *dt_out = __ddiv_rn(cfl, m);
+    if (nonphysical_out) *nonphysical_out = (int)(__ldcg(&hdr[1]) & 1u);
+    hdr[0] = 0u;  // left clean for the next call (the host clears them again before it launches)
+    hdr[1] = 0u;
+  }
+}
+
+}  // namespace mfc
+
+// Device address of static_scratch on `device`, which must be current: asked of the runtime on the first call for that
+// device, remembered afterwards.  The mutex only orders host threads that get here together; it allocates nothing.
+constexpr int MFC_STATIC_MAX_DEVICES = 64;
+static unsigned char* g_static_dev_ptr[MFC_STATIC_MAX_DEVICES] = {};
+static std::mutex g_static_mutex;
+
+static mfc_status static_scratch_on(int device, unsigned char** out) {
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_dev_ptr[device]) {
+    void* ptr = nullptr;
+    CK(cudaGetSymbolAddress(&ptr, mfc::static_scratch));
+    if (!ptr) return fail(MFC_ERR_CUDA, "mfc_cfl_dt_static: cudaGetSymbolAddress returned no address");
+    g_static_dev_ptr[device] = static_cast<unsigned char*>(ptr);
+  }
+  *out = g_static_dev_ptr[device];
+  return MFC_OK;
+}
+
+template <int N, int D>
+static cudaError_t launch_cfl_static(const KP& kp, const double* q, double cfl, unsigned char* scratch, double* dt_out,
+                                     int* nonphysical_out, cudaStream_t stream) {
+  const unsigned nb = (unsigned)((kp.ncells + ST_CPB - 1) / ST_CPB);
+  cfl_static_kernel<N, D><<<nb, PB, 0, stream>>>(kp, q, cfl, scratch, dt_out, nonphysical_out);
+  return cudaGetLastError();
+}
+
+extern "C" mfc_status mfc_cfl_dt_static(const mfc_params* p, const double* q, double cfl, double* dt_out,
+                                        int* nonphysical_out) {
+  if (!p || !q || !dt_out) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: NULL argument");
+  if (p->ndim < 1 || p->ndim > 3) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: ndim must be 1..3");
+  if (p->nfluids < 1 || p->nfluids > MFC_MAX_FLUIDS) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: nfluids must be 1..3");
+  if (!p->gamma || !p->pi_inf) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: gamma/pi_inf NULL");
+  long long cells = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (p->n[d] < 1) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: n[d] must be >= 1");
+    if (d >= p->ndim && p->n[d] != 1) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: n[d] must be 1 for d >= ndim");
+    if (d < p->ndim && !(p->dx[d] > 0.0)) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: dx[d] must be > 0");
+    cells *= p->n[d];
+    if (cells > MFC_STATIC_MAX_CELLS)
+      return fail(MFC_ERR_ARG,
+                  "mfc_cfl_dt_static: grid too large for the built-in scratch array (at most " +
+                      std::to_string(MFC_STATIC_MAX_CELLS) + " cells = " + std::to_string(MFC_STATIC_MAX_BLOCKS) +
+                      " blocks of " + std::to_string(MFC_STATIC_CELLS_PER_BLOCK) +
+                      "); use mfc_init_grid + mfc_cfl_dt, which allocate their own");
+  }
+  for (int i = 0; i < p->nfluids; ++i)
+    if (!(p->gamma[i] > 1.0)) return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: gamma_i must be > 1");
+  int ndev = 0;
+  CK(cudaGetDeviceCount(&ndev));
+  if (p->device < 0 || p->device >= ndev || p->device >= MFC_STATIC_MAX_DEVICES)
+    return fail(MFC_ERR_ARG, "mfc_cfl_dt_static: no such CUDA device");
+  CK(cudaSetDevice(p->device));
+  unsigned char* scratch = nullptr;
+  if (mfc_status s = static_scratch_on(p->device, &scratch)) return s;
+
+  KP kp;
+  std::memset(&kp, 0, sizeof(KP));
+  for (int d = 0; d < 3; ++d) {
+    kp.n[d] = p->n[d];
+    kp.dx[d] = d < p->ndim ? p->dx[d] : 1.0;
+    kp.inv_dx[d] = 1.0 / kp.dx[d];
+  }
+  kp.ncells = cells;
+  for (int i = 0; i < p->nfluids; ++i) {  // as in mfc_init_grid (PAPER.md:117 with eq.(4))
+    kp.G[i] = 1.0 / (p->gamma[i] - 1.0);
+    kp.P[i] = (p->gamma[i] * p->pi_inf[i]) / (p->gamma[i] - 1.0);
+  }
+  cudaStream_t stream = (cudaStream_t)p->stream;
+  // the array keeps whatever the last call left: the counter and the flag must start at zero even if that call died
+  CK(cudaMemsetAsync(scratch, 0, 2 * sizeof(unsigned), stream));
+  struct { int nf, ndim; } sel{p->nfluids, p->ndim};
+  CK(MFC_DISPATCH(&sel, (launch_cfl_static<N, D>(kp, q, cfl, scratch, dt_out, nonphysical_out, stream))));
+  return MFC_OK;
+}
