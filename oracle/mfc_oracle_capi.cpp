@@ -150,8 +150,22 @@ double oracle_kapila_K(const oracle_params* p, double pres, double alpha1, doubl
   return kapila_K<double>(convert<double>(p), pres, alpha1, alpha2);
 }
 
+// p->form selects the evaluation form, as Solver::rhs does: FORM_DIFFERENCE -> hllc_face, FORM_TEXTBOOK -> hllc_face_textbook
 int oracle_hllc_face(const oracle_params* p, int dir, const double* wL, const double* wR, double* F, double* uf) {
+  if (p->form == FORM_TEXTBOOK) return hllc_face_textbook<double>(convert<double>(p), dir, wL, wR, F, uf);
   return hllc_face<double>(convert<double>(p), dir, wL, wR, F, uf);
+}
+
+// O3 typed as PAPER.md:163 prints it (weno5_js_textbook), fp64 and 80-bit
+void oracle_weno5_js_textbook(const double* s, double eps, double* left, double* right) {
+  weno5_js_textbook<double>(s[0], s[1], s[2], s[3], s[4], eps, left, right);
+}
+
+void oracle_weno5_js_textbook_ld(const double* s, double eps, double* left, double* right) {
+  long double l, r;
+  weno5_js_textbook<long double>(s[0], s[1], s[2], s[3], s[4], (long double)eps, &l, &r);
+  *left = double(l);
+  *right = double(r);
 }
 
 void oracle_clamp_cell(const oracle_params* p, double* q) { clamp_cell<double>(convert<double>(p), q); }

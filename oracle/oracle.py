@@ -46,6 +46,8 @@ def lib():
         L.oracle_cfl_dt.argtypes = [pp, dp, C.c_double]; L.oracle_cfl_dt.restype = C.c_double
         L.oracle_weno5_js.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js.restype = None
         L.oracle_weno5_js_ld.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js_ld.restype = None
+        L.oracle_weno5_js_textbook.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js_textbook.restype = None
+        L.oracle_weno5_js_textbook_ld.argtypes = [dp, C.c_double, dp, dp]; L.oracle_weno5_js_textbook_ld.restype = None
         L.oracle_weno5.argtypes = [C.c_int, dp, C.c_double, dp, dp]; L.oracle_weno5.restype = None
         L.oracle_weno5_ld.argtypes = [C.c_int, dp, C.c_double, dp, dp]; L.oracle_weno5_ld.restype = None
         L.oracle_kapila_K.argtypes = [C.POINTER(OracleParams), C.c_double, C.c_double, C.c_double]
@@ -150,10 +152,12 @@ class Oracle:
         return q
 
 
-def weno5_js(s, eps):
+def weno5_js(s, eps, form="difference"):
+    """form: "difference" (weno5_js, reading N2) or "textbook" (weno5_js_textbook, PAPER.md:163 as printed)"""
     s = np.ascontiguousarray(s, dtype=np.float64)
     l, r = C.c_double(), C.c_double()
-    lib().oracle_weno5_js(_dp(s), float(eps), C.byref(l), C.byref(r))
+    fn = {"difference": lib().oracle_weno5_js, "textbook": lib().oracle_weno5_js_textbook}[form]
+    fn(_dp(s), float(eps), C.byref(l), C.byref(r))
     return l.value, r.value
 
 
@@ -173,10 +177,11 @@ def weno5_weights(recon, dr, beta, eps):
     return om
 
 
-def weno5_js_ld(s, eps):
+def weno5_js_ld(s, eps, form="difference"):
     s = np.ascontiguousarray(s, dtype=np.float64)
     l, r = C.c_double(), C.c_double()
-    lib().oracle_weno5_js_ld(_dp(s), float(eps), C.byref(l), C.byref(r))
+    fn = {"difference": lib().oracle_weno5_js_ld, "textbook": lib().oracle_weno5_js_textbook_ld}[form]
+    fn(_dp(s), float(eps), C.byref(l), C.byref(r))
     return l.value, r.value
 
 

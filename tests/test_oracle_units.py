@@ -58,43 +58,52 @@ def test_prim_pure_fluid_closed_form():
     assert np.allclose(w[1], u, rtol=1e-15)
 
 
+# Every pin of O3 (JS weights) and O4 below runs on BOTH instantiations of the reference: the difference form (readings N2 /
+# N3, what the parity bars are measured against) and the textbook form (PAPER.md:163 f = sum omega_r f^(r); PAPER.md:197,
+# 668 F = F_K + S_K (q*_K - q_K)) — the second exists to make the parity claim independent of the evaluation form, so it
+# must stand on the same pins as the first, not on the CUDA path.
+@pytest.fixture(params=["difference", "textbook"])
+def form(request):
+    return request.param
+
+
 # ------------------------------------------------------------------ O3 WENO5-JS
-def test_weno_linear_data_exact():
-    l, r = O.weno5_js([1, 2, 3, 4, 5], 1e-16)
+def test_weno_linear_data_exact(form):
+    l, r = O.weno5_js([1, 2, 3, 4, 5], 1e-16, form=form)
     assert l == pytest.approx(3.5, abs=1e-14) and r == pytest.approx(2.5, abs=1e-14)
-    l, r = O.weno5_js([7, 7, 7, 7, 7], 1e-16)
+    l, r = O.weno5_js([7, 7, 7, 7, 7], 1e-16, form=form)
     assert l == pytest.approx(7.0, rel=4e-16) and r == pytest.approx(7.0, rel=4e-16)  # weights sum to 1 only to an ulp
 
 
-def test_weno_ideal_weights_closed_form():
+def test_weno_ideal_weights_closed_form(form):
     # eps -> infinity switches the nonlinear weights to the ideal ones: the result must be the
     # 5th-order linear reconstruction (2,-13,47,27,-3)/60 (and its mirror) for ANY data
     rng = np.random.default_rng(3)
     for _ in range(50):
         s = rng.normal(size=5)
-        l, r = O.weno5_js(s, 1e30)
+        l, r = O.weno5_js(s, 1e30, form=form)
         cl = np.array([2, -13, 47, 27, -3]) / 60.0
         assert l == pytest.approx(cl @ s, rel=1e-13, abs=1e-14)
         assert r == pytest.approx(cl[::-1] @ s, rel=1e-13, abs=1e-14)
 
 
-def test_weno_candidates_each_reproduce_quadratics():
+def test_weno_candidates_each_reproduce_quadratics(form):
     # cell averages of x^2 on unit cells are i^2 + 1/12; all three smoothness indicators equal 13/3, so
     # the weights are ideal and the face values are the point values (+-1/2)^2 = 1/4
     s = np.array([4, 1, 0, 1, 4]) + 1.0 / 12.0
-    l, r = O.weno5_js(s, 1e-16)
+    l, r = O.weno5_js(s, 1e-16, form=form)
     assert l == pytest.approx(0.25, abs=1e-13) and r == pytest.approx(0.25, abs=1e-13)
     # cubic: x^3 cell averages = i^3 + i/4 ; exact point value at 1/2 is 1/8 for a 5th-order linear scheme
     i = np.arange(-2, 3)
-    l, _ = O.weno5_js(i ** 3 + i / 4.0, 1e30)
+    l, _ = O.weno5_js(i ** 3 + i / 4.0, 1e30, form=form)
     assert l == pytest.approx(0.125, abs=1e-13)
 
 
-def test_weno_eno_property_at_step():
+def test_weno_eno_property_at_step(form):
     # the stencil that avoids the jump wins: values stay at the smooth side's level
-    l, r = O.weno5_js([0, 0, 0, 1, 1], 1e-16)
+    l, r = O.weno5_js([0, 0, 0, 1, 1], 1e-16, form=form)
     assert abs(l) < 1e-12
-    l, r = O.weno5_js([0, 0, 1, 1, 1], 1e-16)
+    l, r = O.weno5_js([0, 0, 1, 1, 1], 1e-16, form=form)
     assert abs(r - 1.0) < 1e-12
     # jump weights against brute-force evaluation of the definition with fractions-like float math
     s = np.array([1.0, 1.0, 1.0, 3.0, 3.5])
@@ -104,16 +113,16 @@ def test_weno_eno_property_at_step():
     eps = 1e-6
     al = np.array([0.1, 0.6, 0.3]) / (np.array(b) + eps) ** 2
     pl = np.array([(2 * s[0] - 7 * s[1] + 11 * s[2]) / 6, (-s[1] + 5 * s[2] + 2 * s[3]) / 6, (2 * s[2] + 5 * s[3] - s[4]) / 6])
-    l, _ = O.weno5_js(s, eps)
+    l, _ = O.weno5_js(s, eps, form=form)
     assert l == pytest.approx((al / al.sum()) @ pl, rel=1e-14)
 
 
-def test_weno_mirror_symmetry():
+def test_weno_mirror_symmetry(form):
     rng = np.random.default_rng(11)
     for _ in range(100):
         s = rng.normal(size=5) * 10 ** rng.uniform(-3, 3)
-        l, r = O.weno5_js(s, 1e-10)
-        l2, r2 = O.weno5_js(s[::-1].copy(), 1e-10)
+        l, r = O.weno5_js(s, 1e-10, form=form)
+        l2, r2 = O.weno5_js(s[::-1].copy(), 1e-10, form=form)
         assert l == pytest.approx(r2, rel=1e-12) and r == pytest.approx(l2, rel=1e-12)
 
 
@@ -143,13 +152,16 @@ def test_weno_difference_form_is_the_textbook_form_and_rounds_to_half_an_ulp():
         l, r = O.weno5_js(s, eps)
         scale = np.abs(s).max()
         assert abs(l - (al / al.sum()) @ pl) <= 2e-14 * scale and abs(r - (ar / ar.sum()) @ pr) <= 2e-14 * scale
+        # the textbook instantiation IS this transcription (same operations up to the order of a sum): a few ulp
+        lt, rt = O.weno5_js(s, eps, form="textbook")
+        assert abs(lt - (al / al.sum()) @ pl) <= 2e-15 * scale and abs(rt - (ar / ar.sum()) @ pr) <= 2e-15 * scale
         if k >= 150:
             l80, r80 = O.weno5_js_ld(s, eps)
             worst_ulp = max(worst_ulp, abs(l - l80) / np.spacing(abs(l80)), abs(r - r80) / np.spacing(abs(r80)))
     assert worst_ulp <= 1.0, worst_ulp
 
 
-def test_weno_fifth_order_on_cell_averaged_sine():
+def test_weno_fifth_order_on_cell_averaged_sine(form):
     # brute-force refinement: error of the face value against the exact point value
     errs = []
     Ns = [16, 32, 64, 128]
@@ -160,7 +172,7 @@ def test_weno_fifth_order_on_cell_averaged_sine():
         e = 0.0
         for i in range(N):
             s = avg[[(i + k) % N for k in range(-2, 3)]]
-            l, r = O.weno5_js(s, 1e-6)
+            l, r = O.weno5_js(s, 1e-6, form=form)
             e = max(e, abs(l - (2 + np.sin(2 * np.pi * xe[i + 1]))), abs(r - (2 + np.sin(2 * np.pi * xe[i]))))
         errs.append(e)
     rates = np.log2(np.array(errs[:-1]) / np.array(errs[1:]))
@@ -198,9 +210,9 @@ def _rand_prim(case, rng, mach=0.3):
 
 
 @pytest.mark.parametrize("ndim,nfluids", [(1, 1), (2, 2), (3, 2), (3, 3)])
-def test_hllc_consistency(ndim, nfluids):
+def test_hllc_consistency(ndim, nfluids, form):
     case = small_case(ndim, nfluids)
-    orc = O.Oracle(case)
+    orc = O.Oracle(case, form=form)
     rng = np.random.default_rng(5)
     for d in range(ndim):
         for _ in range(20):
@@ -212,9 +224,9 @@ def test_hllc_consistency(ndim, nfluids):
             assert uf == pytest.approx(w[nfluids + d], rel=1e-12, abs=1e-12)
 
 
-def test_hllc_supersonic_upwinding():
+def test_hllc_supersonic_upwinding(form):
     case = small_case(3, 2, gamma=(1.4, 1.67), pi_inf=(0.0, 0.0))
-    orc = O.Oracle(case)
+    orc = O.Oracle(case, form=form)
     rng = np.random.default_rng(9)
     for d in range(3):
         wL, wR = _rand_prim(case, rng), _rand_prim(case, rng)
@@ -228,10 +240,10 @@ def test_hllc_supersonic_upwinding():
             assert uf == (wL2 if up == "L" else wR2)[2 + d]
 
 
-def test_hllc_stationary_contact_exact():
+def test_hllc_stationary_contact_exact(form):
     # u = 0, equal p, jump in density AND in fluid: the contact must be resolved exactly
     case = small_case(2, 2)
-    orc = O.Oracle(case)
+    orc = O.Oracle(case, form=form)
     p = 1.0e5
     wL = np.array([1.0e-6 * 1.0, (1 - 1e-6) * 1000.0, 0.0, 0.0, p, 1.0e-6, 1 - 1e-6])
     wR = np.array([(1 - 1e-6) * 1.0, 1e-6 * 1000.0, 0.0, 0.0, p, 1 - 1e-6, 1e-6])
@@ -242,9 +254,9 @@ def test_hllc_stationary_contact_exact():
         assert np.array_equal(F, exp), F
 
 
-def test_hllc_mirror_symmetry():
+def test_hllc_mirror_symmetry(form):
     case = small_case(3, 2)
-    orc = O.Oracle(case)
+    orc = O.Oracle(case, form=form)
     rng = np.random.default_rng(21)
     N = 2
     for d in range(3):
@@ -259,14 +271,14 @@ def test_hllc_mirror_symmetry():
             assert ufm == pytest.approx(-uf, rel=1e-11, abs=1e-9)
 
 
-def test_hllc_matches_textbook_form_single_ideal_gas():
+def test_hllc_matches_textbook_form_single_ideal_gas(form):
     """For one ideal gas the flux must equal the textbook HLLC written in its OTHER standard form,
     F*_K = [S*(S_K U_K - F_K) + S_K (p_K + rho_K (S_K-u_K)(S*-u_K)) D*] / (S_K - S*),  D* = (0, n, S*)
     (ref. [31] of the paper), with the same Davis wave speeds — catches a dropped or
     mis-signed term in the star state."""
     g = 1.4
     case = small_case(3, 1, gamma=(g,), pi_inf=(0.0,))
-    orc = O.Oracle(case)
+    orc = O.Oracle(case, form=form)
     rng = np.random.default_rng(2)
     seen = set()
     for trial in range(400):
@@ -298,6 +310,46 @@ def test_hllc_matches_textbook_form_single_ideal_gas():
             rho_up = rL if Ss >= 0 else rR
             assert uf == pytest.approx(ref[0] / rho_up, rel=1e-11, abs=1e-11)
     assert seen == {"L", "*L", "*R", "R"}
+
+
+def test_hllc_textbook_and_difference_forms_agree_on_stiffened_gas_faces():
+    """Random two- and three-fluid faces with water (pi_inf = 6e8) in them, all four branches: the flux typed as
+    F_K + S_K (q*_K - q_K) with the star state of PAPER.md:668 formed first equals the flux of reading N3 (chi - 1 formed
+    directly) up to the rounding of the subtraction q*_K - q_K, i.e. a few ulp of S_K q_K — with stiff water a dropped term
+    in the star energy is ten orders of magnitude above that."""
+    rng = np.random.default_rng(31)
+    seen = set()
+    for nfl in (2, 3):
+        case = small_case(3, nfl)
+        d_orc, t_orc = O.Oracle(case), O.Oracle(case, form="textbook")
+        N, D = nfl, 3
+        for trial in range(300):
+            d = trial % 3
+            wL, wR = _rand_prim(case, rng, mach=rng.choice([0.1, 1.0, 8.0])), _rand_prim(case, rng, mach=rng.choice([0.1, 1.0, 8.0]))
+            if trial % 4 == 0:      # supersonic either way: the non-star branches
+                s = rng.choice([-1.0, 1.0]) * 9000.0
+                wL[N + d], wR[N + d] = s, 1.05 * s
+            Fd, ufd, bd = d_orc.hllc_face(d, wL, wR)
+            Ft, uft, bt = t_orc.hllc_face(d, wL, wR)
+            assert bd == 0 and bt == 0
+            # magnitudes: |S| <= |u| + c, q_K the conserved state of the two sides
+            smax, qmag = 0.0, np.zeros(case.neq)
+            for w in (wL, wR):
+                rho = w[:N].sum()
+                Gam = sum(w[N + D + 1 + i] / (case.gamma[i] - 1) for i in range(N))
+                Pi = sum(w[N + D + 1 + i] * case.gamma[i] * case.pi_inf[i] / (case.gamma[i] - 1) for i in range(N))
+                c = np.sqrt(((Gam + 1) * w[N + D] + Pi) / (Gam * rho))
+                smax = max(smax, abs(w[N + d]) + c)
+                qc = w.copy()
+                qc[N:N + D] = rho * np.abs(w[N:N + D]) + rho * c
+                qc[N + D] = Gam * w[N + D] + Pi + 0.5 * rho * (w[N:N + D] @ w[N:N + D])
+                qmag = np.maximum(qmag, np.abs(qc))
+            tol = 1e-13 * np.maximum(np.abs(Fd), smax * qmag)
+            assert np.all(np.abs(Ft - Fd) <= tol), (trial, Ft - Fd, tol)
+            assert abs(uft - ufd) <= 1e-13 * smax
+            pure = ufd == wL[N + d] or ufd == wR[N + d]     # outside the fan the face velocity is the upwind side's own
+            seen.add(("pure" if pure else "star", ufd >= 0))
+    assert len(seen) == 4, seen
 
 
 # ------------------------------------------------------------------ A9, A10 (definitions only: parity unpinned by the paper)
