@@ -123,8 +123,10 @@ mfc_status mfc_prim_from_cons(mfc_grid *g, const double *q, double *w);
 mfc_status mfc_rhs(mfc_grid *g, const double *q, double *rhs);
 
 /* As mfc_rhs but only the directions whose bit is set in dir_mask (bit d = direction d) contribute;
- * cells keep 0 from the other directions.  The viscous rates (eta > 0) are part of the result only for dir_mask == 7,
- * whatever the number of dimensions.  Exists so that each directional sweep can be tested alone. */
+ * cells keep 0 from the other directions.  dir_mask must be 1..7 (else MFC_ERR_ARG).  The viscous rates (eta > 0) are part
+ * of the result only for dir_mask == 7, whatever the number of dimensions; on a handle with eta > 0 any other mask that
+ * covers all of the grid's directions (3 in 2-D, 1 in 1-D, ...) is refused with MFC_ERR_ARG rather than answered without
+ * them.  Exists so that each directional sweep can be tested alone. */
 mfc_status mfc_rhs_dirs(mfc_grid *g, const double *q, double *rhs, int dir_mask);
 
 /* One SSP-RK3 step of size dt (the three-stage formula), in place on q, with the A10
@@ -237,6 +239,14 @@ mfc_status mfc_get_profile(mfc_grid *g, int kernel_class, double *total_ms_host,
  * All pointers device; async. */
 mfc_status mfc_weno5_values(mfc_grid *g, const double *stencils, long long count, double *left, double *right);
 mfc_status mfc_hllc_faces(mfc_grid *g, int dir, const double *wL, const double *wR, long long count, double *F, double *uf);
+
+/* Unit-level entry point of the square root of a ratio the Riemann solver uses for the face sound speed,
+ * c = sqrt(cn / (Gamma rho)) (A5): out[t] = a[t] * rsqrt(a[t] b[t]) refined once, as in the sweeps, and (seed_out not NULL)
+ * the raw hardware rsqrt(a[t] b[t]) the refinement starts from.  Valid where the PRODUCT a b is a normal double that
+ * neither overflows nor is flushed to zero (about 1e-307 < a b < 1e308; for the sound speed a b ~ p Gamma rho, 1e3..1e14
+ * in SI units); a product that underflows makes the sweeps flag the face as non-physical, one that overflows gives 0.
+ * All pointers device, count doubles each; async. */
+mfc_status mfc_sqrt_ratio_values(mfc_grid *g, const double *a, const double *b, long long count, double *out, double *seed_out);
 
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 long long mfc_launch_count(const mfc_grid *g);

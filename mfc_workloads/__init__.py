@@ -44,6 +44,8 @@ class Case:
     model: str = "allaire"   # volume-fraction equation: "allaire" (no K div u) or "kapila" (eq. 5; two fluids)
     eta: float = 0.0         # uniform shear viscosity of PAPER.md eq.(1); 0 = inviscid (all five configurations)
     weno: str = "js"         # nonlinear weights: "js" (BASELINE.json), "m" (mapped), "z"
+    shock_x: float = -1.0    # config 5 only: position of the incident shock; < 0 = the configuration's own (0.2).  Tests move it
+                             # next to the droplet (surface at x = 0.30) to sample a state in which the two already interact
 
     @property
     def neq(self):
@@ -206,7 +208,7 @@ def _build_shock_droplet_3d(case):
     a_l = np.clip(np.minimum(np.broadcast_to(slab, case.shape[1:]), 1.0 - a_w - f), f, None)
     a_a = 1.0 - a_w - a_l
     rho1, u1, p1 = _normal_shock(1.4, 1.5, 1.0, 1.0e5)
-    post = np.broadcast_to(X < 0.2, case.shape[1:])
+    post = np.broadcast_to(X < (case.shock_x if case.shock_x >= 0.0 else 0.2), case.shape[1:])
     rho_air = np.where(post, rho1, 1.0)
     ux = np.where(post, u1, 0.0)
     p = np.where(post, p1, 1.0e5)

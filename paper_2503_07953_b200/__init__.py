@@ -20,7 +20,8 @@ EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "m
            "mfc_rhs_dirs", "mfc_rk3_step", "mfc_rk3_steps", "mfc_cfl_dt", "mfc_check", "mfc_rhs_host",
            "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
            "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error", "mfc_set_halo", "mfc_rk3_stage",
-           "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64", "mfc_rk3_stage_parts", "mfc_cfl_dt_static")
+           "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64", "mfc_rk3_stage_parts", "mfc_cfl_dt_static",
+           "mfc_sqrt_ratio_values")
 STATIC_MAX_CELLS = 2048 * 16384  # MFC_STATIC_MAX_CELLS of include/mfc_b200.h
 
 
@@ -85,6 +86,7 @@ def lib():
         L.mfc_stage_input.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_void_p)]
         L.mfc_pack_halo.argtypes = [vp, dp, C.c_int, dp, dp]
         L.mfc_measure_fp64.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.mfc_sqrt_ratio_values.argtypes = [vp, dp, dp, C.c_longlong, dp, dp]
         L.mfc_cfl_dt_static.argtypes = [C.POINTER(MfcParams), dp, C.c_double, dp, dp]
         _lib = L
     return _lib
@@ -273,6 +275,11 @@ class Grid:
         n = uf.numel()
         _ck(lib().mfc_hllc_faces(self._h, int(direction), _dev_ptr(wL, n * self.neq), _dev_ptr(wR, n * self.neq), n,
                                  _dev_ptr(F, n * self.neq), _dev_ptr(uf, n)))
+
+    def sqrt_ratio_values(self, a, b, out, seed_out=None):
+        n = out.numel()
+        _ck(lib().mfc_sqrt_ratio_values(self._h, _dev_ptr(a, n), _dev_ptr(b, n), n, _dev_ptr(out, n),
+                                        _dev_ptr(seed_out, n) if seed_out is not None else None))
 
     def set_halo(self, halo_lo, halo_hi):
         """halo_lo / halo_hi: CUDA float64 tensors of neq*3*plane elements ([v][layer][plane]) or None; kept alive here"""

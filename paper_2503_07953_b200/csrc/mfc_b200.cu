@@ -596,6 +596,21 @@ __global__ void __launch_bounds__(PB) hllc_unit_kernel(const __grid_constant__ K
   uf[t] = u;
 }
 
+// fsqrt_ratio(a, a b) as the Riemann solver calls it for the face sound speed (a = cn, b = Gamma rho), and the raw
+// hardware seed rsqrt(a b) it starts from — so that a test can measure both against the correctly rounded sqrt(a / b).
+__global__ void __launch_bounds__(PB) sqrt_ratio_unit_kernel(const double* __restrict__ a, const double* __restrict__ b,
+                                                             long long count, double* out, double* seed_out) {
+  const long long t = (long long)blockIdx.x * PB + threadIdx.x;
+  if (t >= count) return;
+  const double ct = a[t] * b[t];
+  out[t] = fsqrt_ratio(a[t], ct);
+  if (seed_out) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(ct));
+    seed_out[t] = y;
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ viscous terms
 // O8 (eqs.(1),(2); reading A22): T = 2 eta (D - tr(D) I/3) with one uniform eta, second-order
 // central differences at face centres.  Two pointwise kernels, bound by HBM/L2, run BEFORE the sweeps of an RHS evaluation:
@@ -1282,6 +1297,11 @@ mfc_status mfc_prim_from_cons(mfc_grid* g, const double* q, double* w) {
 mfc_status mfc_rhs_dirs(mfc_grid* g, const double* q, double* rhs, int dir_mask) {
   if (!g || !q || !rhs) return fail(MFC_ERR_ARG, "mfc_rhs: NULL argument");
   if (q == rhs) return fail(MFC_ERR_ARG, "mfc_rhs: q and rhs must not alias");
+  if (dir_mask < 1 || dir_mask > 7) return fail(MFC_ERR_ARG, "mfc_rhs_dirs: dir_mask must be 1..7 (bit d = direction d)");
+  // the viscous rates belong to the whole RHS, which is spelt 7 whatever the number of dimensions: a mask that names all of
+  // this grid's directions in another way (3 on a 2-D grid) would silently come back inviscid — refuse it instead
+  if (g->kp.eta > 0.0 && dir_mask != 7 && (dir_mask & ((1 << g->ndim) - 1)) == (1 << g->ndim) - 1)
+    return fail(MFC_ERR_ARG, "mfc_rhs_dirs: with eta > 0 the full RHS (viscous rates included) is dir_mask 7; a partial mask must leave a direction of the grid out");
   if (halo_missing(g)) return fail(MFC_ERR_ARG, "mfc_rhs: MFC_BC_HALO without mfc_set_halo");
   if (mfc_status s = use_device(g)) return s;
   CK(MFC_DISPATCH_W(g, (launch_rhs<N, D, WV>(g, q, rhs, dir_mask))));
@@ -1486,6 +1506,19 @@ mfc_status mfc_hllc_faces(mfc_grid* g, int dir, const double* wL, const double* 
   if (mfc_status s = use_device(g)) return s;
   if (count == 0) return MFC_OK;
   CK(MFC_DISPATCH(g, (launch_hllc_unit<N, D>(g, dir, wL, wR, count, F, uf))));
+  return MFC_OK;
+}
+
+mfc_status mfc_sqrt_ratio_values(mfc_grid* g, const double* a, const double* b, long long count, double* out, double* seed_out) {
+  if (!g || !a || !b || !out) return fail(MFC_ERR_ARG, "mfc_sqrt_ratio_values: NULL argument");
+  if (count < 0) return fail(MFC_ERR_ARG, "mfc_sqrt_ratio_values: count < 0");
+  if (count == 0) return MFC_OK;
+  if (mfc_status s = use_device(g)) return s;
+  {
+    Scope sc(g, MFC_K_PRIM);
+    sqrt_ratio_unit_kernel<<<(unsigned)((count + PB - 1) / PB), PB, 0, g->stream>>>(a, b, count, out, seed_out);
+  }
+  CK(cudaGetLastError());
   return MFC_OK;
 }
 

@@ -60,9 +60,15 @@ __device__ __forceinline__ double kapila_K(const KP& kp, double p, double a1, do
   return ((a1 * a2) * (A2 - A1)) * frcp(den);
 }
 
-// sqrt(a/b) for a b > 0 without forming the quotient: a * rsqrt(a b), the hardware rsqrt seed y (relative error e' ~ 2^-23)
-// refined by one cubically convergent step y (1 + e/2 + 3 e^2/8), e = 1 - (a b) y^2  ->  ~2^-68 before the final rounding.
-// 8 FP64 instructions and one MUFU where reciprocal + multiply + square root took 12 and two.
+// sqrt(a/b) for a b > 0 without forming the quotient: a * rsqrt(a b), the hardware rsqrt seed y refined by one cubically
+// convergent step y (1 + e/2 + 3 e^2/8), e = 1 - (a b) y^2.  Measured on B200 (mfc_sqrt_ratio_values,
+// tests/test_gpu_parity.py::test_sqrt_ratio_unit_entry_point, 2^18 pairs over 280 decades of a b): the seed's relative error
+// is at most 2^-20.1 (rsqrt.approx.ftz.f64 looks at the upper half of its operand), so e <= 2^-19 and the neglected e^3 term
+// is ~2^-59; with the roundings of t y, the two FMAs and the final product the result is within 1.86 ulp of the correctly
+// rounded sqrt(a/b).  8 FP64 instructions and one MUFU where reciprocal + multiply + square root took 12 and two.
+// RANGE: the PRODUCT t = a b must be a normal double — it has half the exponent range of the quotient.  t flushed to zero
+// (ftz) fails the callers' `ct > 0` test and the face is flagged non-physical; t overflowing to +inf would pass that test
+// and give 0.  For the sound speed t ~ p Gamma rho, 1e3..1e14 in SI units (1e-2..1e3 nondimensional): far inside.
 __device__ __forceinline__ double fsqrt_ratio(double a, double t /* = a b */) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(t));

@@ -10,9 +10,15 @@ exchanges of neq*3*plane doubles per end and one scalar MIN all-reduce for dt.  
 
 This module is host plumbing only (partition, neighbours, buffers, the exchange); all arithmetic runs in the kernels.
 """
+import os
 from dataclasses import replace
 
 from . import BC_EXTRAP, BC_HALO, BC_PERIODIC, Grid
+
+# MFC_SLAB_SYNC=1: host-synchronise behind the packing and behind the transfers instead of relying on stream events alone.
+# The event ordering of the NCCL branch has been read, not run (no two-GPU box so far): this is the safe way out if a
+# two-process run shows halos read before they have landed.
+SYNC_FALLBACK = os.environ.get("MFC_SLAB_SYNC", "0") == "1"
 
 
 def partition(n_last, world):
@@ -111,16 +117,30 @@ class Slab:
         if self.below is None and self.above is None:
             return []
         import torch
+        cur = torch.cuda.current_stream(self.stream.device)
+        if cur != self.stream:
+            # whatever produced q was enqueued on the caller's current stream: the handle's stream (packing, sweeps) follows it
+            ev = torch.cuda.Event()
+            ev.record(cur)
+            self.stream.wait_event(ev)
         self.pack(q, stage)
-        if not (self.below == self.rank and self.above == self.rank):
-            # the packed buffers must be complete before NCCL reads them: NCCL's stream waits for the CURRENT stream when the
-            # transfers are posted, so the current stream is made to wait for an event recorded behind the packing — the
-            # host is not stalled (no synchronize; three per step in round 1)
-            cur = torch.cuda.current_stream(self.stream.device)
-            if cur != self.stream:
-                ev = torch.cuda.Event()
-                ev.record(self.stream)
-                cur.wait_event(ev)
+        if SYNC_FALLBACK:
+            self.stream.synchronize()
+        if self.below == self.rank and self.above == self.rank:
+            # one periodic slab, its own neighbour: the two local copies run on the handle's stream, between the packing and
+            # the sweep that reads the halos — ordered by the stream itself, whatever the caller's current stream is
+            with torch.cuda.stream(self.stream):
+                exchange(self.send_lo, self.send_hi, self.halo_lo, self.halo_hi, self.rank, self.below, self.above,
+                         self.dist, self.group, wait=False)
+            self.exchanges += 1
+            return []
+        # the packed buffers must be complete before NCCL reads them: NCCL's stream waits for the CURRENT stream when the
+        # transfers are posted, so the current stream is made to wait for an event recorded behind the packing — the
+        # host is not stalled (no synchronize; three per step in round 1)
+        if cur != self.stream:
+            ev = torch.cuda.Event()
+            ev.record(self.stream)
+            cur.wait_event(ev)
         works = exchange(self.send_lo, self.send_hi, self.halo_lo, self.halo_hi, self.rank, self.below, self.above,
                          self.dist, self.group, wait=False)
         self.exchanges += 1
@@ -150,6 +170,8 @@ class Slab:
         for w in works:
             w.wait()
         cur = torch.cuda.current_stream(self.stream.device)
+        if SYNC_FALLBACK:
+            cur.synchronize()
         if cur != self.stream:
             ev = torch.cuda.Event()
             ev.record(cur)

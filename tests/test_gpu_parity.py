@@ -10,12 +10,13 @@ import pytest
 
 import mfc_workloads as W
 from oracle import oracle as O
-from parity_norm import group_noise, rel_err
+from parity_norm import case_t2_rows, group_noise, rel_err, rel_err_report, t2_rows, var_names
 
 pytestmark = pytest.mark.gpu
 
 RHS_TOL = 1e-12
 STEP_TOL = 1e-9
+ADJUDICATION_FACTOR = 2.0  # test_rhs_agrees_with_textbook_form_oracle; measured worst 1.60 (config 2, momentum), 0.9-1.0 elsewhere
 
 
 @pytest.fixture(scope="module")
@@ -101,7 +102,7 @@ def test_rhs_rough_state_all_directions(torch, mfc, ndim, nfluids, n, bc):
     ref, noise = oracle_rhs_with_noise(case, q)
     got = gpu_rhs(torch, mfc, case, q)
     # one fluid: alpha == 1 and d(alpha)/dt is analytically zero — the volume-fraction group of the reference is rounding noise
-    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None)
+    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None, t2_rows(nfluids, ndim))
     assert worst <= RHS_TOL, per
 
 
@@ -149,7 +150,7 @@ def test_rhs_configs(torch, mfc, index, n):
     # configs 1, 3, 5 at t = 0: d(alpha)/dt is analytically zero (alpha == 1; alpha uniform wherever the
     # fluid moves, the bubble / droplet being at rest ahead of the shock): the volume-fraction group is
     # allowed the reference's own rounding noise (parity_norm).  configs 2 and 4 are held to the bare bar.
-    worst, per = rel_err(got, ref, case.nfluids, case.ndim, None if index in (2, 4) else noise)
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim, None if index in (2, 4) else noise, case_t2_rows(case))
     assert worst <= RHS_TOL, per
 
 
@@ -165,7 +166,7 @@ def test_rhs_host_entry_point_matches_device_entry_point(torch, mfc):
 
 # ------------------------------------------------------------------ against the paper's text in its textbook form
 @pytest.mark.parametrize("index,n", [(2, None), (3, 128), (4, 48), (5, 40), ("rough23", (33, 18, 11)), ("rough33", (40, 9, 13))])
-def test_rhs_agrees_with_textbook_form_oracle(torch, mfc, index, n):
+def test_rhs_agrees_with_textbook_form_oracle(torch, mfc, capsys, index, n):
     """The first oracle writes WENO5-JS and HLLC in the evaluation forms N2 / N3, the forms the kernels use
     too.  This test makes the parity claim independent of that choice: the oracle's second instantiation types the same two
     definitions as the paper prints them (f = sum omega_r f^(r); F = F_K + S_K (q*_K - q_K)).
@@ -188,6 +189,21 @@ def test_rhs_agrees_with_textbook_form_oracle(torch, mfc, index, n):
         scale = np.abs(t64[v]).max() if not (case.nfluids <= v < case.nfluids + case.ndim) else \
             np.abs(t64[case.nfluids:case.nfluids + case.ndim]).max()
         assert np.abs(got[v] - t64[v]).max() <= 4.0 * noise[v] + RHS_TOL * max(scale, 1e-300), (v, noise[v])
+    # The 80-bit evaluation of the paper's text as the adjudicator: per variable, how far each of the
+    # three fp64 evaluations — the textbook form, the difference form, the kernels — lies from it.  The kernels are about
+    # as close to the exact evaluation of the printed formulas as the printed formulas in fp64 are.
+    o64 = O.Oracle(case).rhs(q)
+    names = var_names(case.nfluids, case.ndim)
+    report, factor = {}, 0.0
+    for v in range(case.neq):
+        d_gpu, d_t, d_o = (float(np.abs(x[v] - t80[v]).max()) for x in (got, t64, o64))
+        report[names[v]] = ("gpu %.2e" % d_gpu, "textbook64 %.2e" % d_t, "difference64 %.2e" % d_o)
+        if max(d_t, d_o) > 0.0:
+            factor = max(factor, d_gpu / max(d_t, d_o))
+        assert d_gpu <= ADJUDICATION_FACTOR * max(d_t, d_o), (names[v], report[names[v]])
+    with capsys.disabled():
+        print(f"\n[adjudication by the 80-bit textbook evaluation, {case.name} {case.n}] worst max|gpu - t80| / "
+              f"max(max|t64 - t80|, max|o64 - t80|) = {factor:.2f}; distances to t80 per variable: {report}")
 
 
 # ------------------------------------------------------------------ full-size parity (the bench launch configurations)
@@ -207,8 +223,8 @@ def test_rhs_full_size_config3_elementwise(torch, mfc):
     q = W.initial_state(case)
     ref, noise = oracle_rhs_with_noise(case, q)
     got = gpu_rhs(torch, mfc, case, q)
-    worst, per = rel_err(got, ref, case.nfluids, case.ndim, noise)
-    assert worst <= RHS_TOL, per
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim, noise, case_t2_rows(case))
+    assert worst <= RHS_TOL, rel_err_report(got, ref, case.nfluids, case.ndim, noise, case_t2_rows(case))
 
 
 def _sampled_box_parity(torch, mfc, case, q, boxes, core):
@@ -240,7 +256,9 @@ def _sampled_box_parity(torch, mfc, case, q, boxes, core):
         gots.append(got.cpu().numpy().reshape(case.neq, -1))
     g.close()
     got, ref, ld = np.concatenate(gots, 1), np.concatenate(refs, 1), np.concatenate(lds, 1)
-    return rel_err(got, ref, case.nfluids, case.ndim, group_noise(ref, ld, case.nfluids, case.ndim))
+    noise, rows = group_noise(ref, ld, case.nfluids, case.ndim), case_t2_rows(case)
+    print("[sampled boxes] per variable (with allowance, without, 4 n64/scale, allowed):", rel_err_report(got, ref, case.nfluids, case.ndim, noise, rows))
+    return rel_err(got, ref, case.nfluids, case.ndim, noise, rows)
 
 
 def test_rhs_full_size_config5_sampled(torch, mfc):
@@ -302,14 +320,18 @@ def test_advance_full_size_config3_elementwise(torch, mfc):
 
 def test_advance_full_size_config5_sampled(torch, mfc, capsys):
     """One CFL + RK3 step of config 5 at the largest n the host holds (512 when there is memory for the 10.7 GB input),
-    compared on sampled 16^3 boxes: the oracle steps a sub-box cut out of q with a 9-cell rim (three stages of a 3-cell
-    stencil), with the time step of the full grid."""
-    import psutil
+    compared on sampled 16^3 boxes: the reference steps a sub-box cut out of q with a 9-cell rim (three stages of a 3-cell
+    stencil), with the time step of the full grid.  The incident shock is moved from x = 0.2 to x = 0.31, where it already
+    cuts the droplet's surface (x >= 0.30): at the configuration's own t = 0 everything but the shock plane is at rest
+    with uniform p, L = 0 there, and a step would be compared mostly on cells that never move.  More than half of the
+    boxes sit on the shock plane (in the free stream, on the droplet's cap, where the plane meets the domain's y and z
+    ends).  A box that touches an end of the domain is cut AT that end, so that the sub-box's own extrapolation boundary
+    is the domain's (rebuilt from the stage state in every stage, as on the full grid), not a band of duplicated cells
+    evolving as if interior."""
+    psutil = pytest.importorskip("psutil")
     avail = psutil.virtual_memory().available
     n = 512 if avail > 40e9 else 320
-    if avail > 40e9:
-        assert n == 512
-    case = W.config(5, n=n)
+    case = replace(W.config(5, n=n), shock_x=0.31)
     q = W.initial_state(case)
     g = mfc.Grid.from_case(case)
     qd = torch.from_numpy(q).cuda()
@@ -317,34 +339,49 @@ def test_advance_full_size_config5_sampled(torch, mfc, capsys):
     g.rk3_step(qd, dt)
     g.check()
     rng = np.random.default_rng(3)
-    at = lambda x, y, z: (int(x * n), int(y * n), int(z * n))
     core, rim = 16, 9
-    boxes = [at(0.2, 0.5, 0.5), at(0.19, 0.1, 0.9), at(0.3, 0.5, 0.5), at(0.45, 0.35, 0.5), at(0.58, 0.5, 0.5),
-             at(0.7, 0.2, 0.3), at(0.84, 0.7, 0.6), (0, 0, 0), (n - core, n - core, n - core), (0, n // 2, n - core)]
-    boxes += [tuple(int(v) for v in rng.integers(0, n - core, 3)) for _ in range(4)]
+    xs = int(0.31 * n) - core // 2    # boxes that straddle the shock plane: all 16 planes lie within 9 cells of it
+    at = lambda y, z: (int(y * n), int(z * n))
+    boxes = [(xs,) + at(0.5, 0.5), (xs,) + at(0.47, 0.53), (xs,) + at(0.42, 0.5), (xs,) + at(0.5, 0.6),   # droplet cap
+             (xs,) + at(0.1, 0.9), (xs,) + at(0.8, 0.25), (xs, 0, n - core), (xs, n - core, 0), (xs, 0, n // 2),  # free stream, ends
+             (int(0.45 * n), int(0.35 * n), int(0.5 * n)), (int(0.7 * n), int(0.2 * n), int(0.3 * n)),  # droplet side, slab face
+             (0, 0, 0), (n - core, n - core, n - core)]
+    boxes += [tuple(int(v) for v in rng.integers(0, n - core, 3)) for _ in range(2)]
     gots, refs, olds = [], [], []
     for lo3 in boxes:
-        idx = [np.clip(np.arange(lo3[d] - rim, lo3[d] + core + rim), 0, n - 1) for d in range(3)]  # extrapolation ends
+        start = [max(lo3[d] - rim, 0) for d in range(3)]
+        idx = [np.arange(start[d], min(lo3[d] + core + rim, n)) for d in range(3)]
         sub = np.ascontiguousarray(q[:, idx[2][:, None, None], idx[1][None, :, None], idx[0][None, None, :]])
         nn = tuple(len(idx[d]) for d in range(3))
         scase = W.Case("box", 3, nn, case.dx, case.nfluids, case.gamma, case.pi_inf, (W.BC_EXTRAP,) * 3, (W.BC_EXTRAP,) * 3,
                        weno_eps=case.weno_eps, alpha_floor=case.alpha_floor, clamp=case.clamp)
-        cut = (slice(None), slice(rim, rim + core), slice(rim, rim + core), slice(rim, rim + core))
+        off = [lo3[d] - start[d] for d in range(3)]
+        cut = (slice(None), slice(off[2], off[2] + core), slice(off[1], off[1] + core), slice(off[0], off[0] + core))
         olds.append(sub[cut].reshape(case.neq, -1).copy())
         orc = O.Oracle(scase)
         orc.rk3_step(sub, dt)
         assert orc.bad == 0
         refs.append(sub[cut].reshape(case.neq, -1))
-        gi = [torch.as_tensor(idx[d][rim:rim + core], device="cuda") for d in range(3)]
+        gi = [torch.arange(lo3[d], lo3[d] + core, device="cuda") for d in range(3)]
         got = qd.view(case.shape)[:, gi[2][:, None, None], gi[1][None, :, None], gi[0][None, None, :]]
         gots.append(got.cpu().numpy().reshape(case.neq, -1))
     g.close()
     got, ref, old = np.concatenate(gots, 1), np.concatenate(refs, 1), np.concatenate(olds, 1)
     worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    moved = float(np.any(ref != old, axis=0).mean())
+    # the increment q^{n+1} - q^n against its own size, variable by variable (as _advance_vs_oracle does at 256^3)
+    _, inc_per = rel_err(got - old, ref - old, case.nfluids, case.ndim)
     with capsys.disabled():
-        print(f"\n[config 5 step parity] n = {n} ({avail / 1e9:.0f} GB of host memory available), {len(boxes)} boxes, worst e_v = {worst:.2e}")
+        print(f"\n[config 5 step parity] n = {n} ({avail / 1e9:.0f} GB of host memory available), {len(boxes)} boxes, "
+              f"{100 * moved:.0f} % of the sampled cells moved, worst e_v = {worst:.2e}, increments: {inc_per}")
     assert worst <= 1e-12, per
-    assert not np.array_equal(got, old)  # the step did move the sampled cells
+    assert moved >= 0.5, moved          # the sample is not made of cells at rest
+    # every variable's increment against its own size, at the one-RHS bar (measured: 3.5e-14).  The one row without a scale of
+    # its own is the volume fraction of the light gas: in the shocked region it sits at the floor (1e-6, the A10 clamp
+    # holds it there) and its largest increment over the sample is ~1e-10 absolute — it is held by the state bar above
+    trace = "alpha3"
+    assert max(v for k, v in inc_per.items() if k != trace) <= 1e-12, inc_per
+    assert inc_per[trace] <= 1e-4, inc_per
 
 
 @pytest.mark.parametrize("seg", [(64, 64, 64), (30, 8, 8), (1000, 1000, 1000), (62, 9, 11), (7, 3, 2)])
@@ -513,6 +550,21 @@ def test_argument_errors(torch, mfc):
         mfc.Grid(2, (8, 8, 2), (1, 1, 1), (1.4,), (0.0,), (0,) * 3, (0,) * 3)
     with pytest.raises(mfc.MfcError):
         mfc.Grid(1, (8, 1, 1), (1, 1, 1), (1.4,), (0.0,), (0, 0, 0), (1, 0, 0))
+    # dir_mask: 1..7 only; on a viscous handle a mask that names all of the grid's directions must be spelt 7 (the viscous
+    # rates belong to the whole RHS) — anything else is refused, not answered inviscid
+    r = torch.full_like(q, 5.0)
+    for bad_mask in (0, 8, 15, -1):
+        with pytest.raises(mfc.MfcError) as e:
+            g.rhs_dirs(q, r, bad_mask)
+        assert e.value.status == mfc.MFC_ERR_ARG
+    gv = mfc.Grid.from_case(replace(case, eta=1.0))
+    for bad_mask in (3,):
+        with pytest.raises(mfc.MfcError) as e:
+            gv.rhs_dirs(q, r, bad_mask)
+        assert e.value.status == mfc.MFC_ERR_ARG and "dir_mask 7" in str(e.value)
+    torch.cuda.synchronize()
+    assert bool((r == 5.0).all())   # argument errors leave the buffers untouched
+    g.rhs_dirs(q.fill_(0.0), r, 3)  # inviscid handle: 3 is simply both directions of a 2-D grid
 
 
 # ------------------------------------------------------------------ unit entry points, one device function at a time
@@ -607,7 +659,7 @@ def test_rhs_rough_state_variant_weights(torch, mfc, ndim, nfluids, n, bc, weno)
     q = rough_state(case, 5 + ndim)
     ref, noise = oracle_rhs_with_noise(case, q)
     got = gpu_rhs(torch, mfc, case, q)
-    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None)
+    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None, t2_rows(nfluids, ndim))
     assert worst <= RHS_TOL, per
 
 
@@ -619,7 +671,7 @@ def test_rhs_configs_variant_weights(torch, mfc, index, n, weno):
     q = W.initial_state(case)
     ref, noise = oracle_rhs_with_noise(case, q)
     got = gpu_rhs(torch, mfc, case, q)
-    worst, per = rel_err(got, ref, case.nfluids, case.ndim, None if index in (2, 4) else noise)  # as in test_rhs_configs
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim, None if index in (2, 4) else noise, case_t2_rows(case))  # as in test_rhs_configs
     assert worst <= RHS_TOL, per
 
 
@@ -699,6 +751,40 @@ def test_kapila_needs_two_fluids(torch, mfc):
     assert e.value.status == mfc.MFC_ERR_ARG
 
 
+# ------------------------------------------------------------------ the square root of a ratio behind the face sound speed
+def test_sqrt_ratio_unit_entry_point(torch, mfc, capsys):
+    """fsqrt_ratio(a, a b) = a rsqrt(a b) with one refinement step (the face sound speed c = sqrt(cn / (Gamma rho)) of the
+    Riemann solver, A5) against sqrt(a / b) evaluated in 80-bit arithmetic and rounded once: within 3 ulp wherever the
+    product a b is a normal double — over the magnitudes of the workloads and over 280 decades of the product."""
+    rng = np.random.default_rng(77)
+    n = 1 << 18
+    la = np.concatenate([rng.uniform(3, 11, n // 2), rng.uniform(-140, 140, n // 2)])   # log10 a: SI pressures; anything
+    lb = np.concatenate([rng.uniform(-3, 5, n // 2), rng.uniform(-140, 140, n // 2)])   # log10 b: Gamma rho; anything
+    a = 10.0 ** la * rng.uniform(1.0, 2.0, n)
+    b = 10.0 ** lb * rng.uniform(1.0, 2.0, n)
+    g = mfc.Grid.from_case(make_case(1, 1, (8, 1, 1), W.BC_EXTRAP))
+    ad, bd = torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda()
+    od, sd = torch.empty_like(ad), torch.empty_like(ad)
+    g.sqrt_ratio_values(ad, bd, od, sd)
+    g.check()
+    got, seed = od.cpu().numpy(), sd.cpu().numpy()
+    L = np.longdouble
+    ref = np.sqrt(L(a) / L(b))
+    ulps = np.abs(L(got) - ref) / np.spacing(ref.astype(np.float64))
+    seed_err = np.abs(L(seed) * np.sqrt(L(a) * L(b)) - 1)
+    with capsys.disabled():
+        print(f"\n[sqrt ratio] max error {float(ulps.max()):.3f} ulp (workload range {float(ulps[:n // 2].max()):.3f}); "
+              f"hardware rsqrt seed: max relative error 2^{float(np.log2(seed_err.max())):.2f}")
+    assert float(ulps.max()) <= 3.0
+    assert float(seed_err.max()) <= 2.0 ** -19   # the refinement cubes it: (2^-19)^3 is far below 2^-53
+    # outside the documented range the product underflows (flushed to zero): the sweeps flag such a face (ct > 0 fails)
+    # instead of using the value; here the entry point just returns what the formula gives — not a finite wrong number
+    tiny = torch.tensor([1e-170, 1e-200], dtype=torch.float64, device="cuda")
+    out = torch.empty_like(tiny)
+    g.sqrt_ratio_values(tiny, tiny.clone(), out)
+    assert not bool(torch.isfinite(out).any())
+
+
 # ------------------------------------------------------------------ slab decomposition (MFC_BC_HALO), several slabs on one GPU
 def _slabs_on_one_gpu(torch, case, q, k):
     """k slabs of the global case, all on this GPU, run one after the other (no rank waits on another); the exchange is
@@ -726,6 +812,42 @@ def _slabs_on_one_gpu(torch, case, q, k):
 def _gather(case, slabs, parts):
     d = case.ndim - 1
     return np.concatenate([p.cpu().numpy() for p in parts], axis=3 - d)
+
+
+@pytest.mark.gpu
+def test_self_exchanging_slab_follows_the_callers_current_stream(torch, mfc):
+    """One periodic slab is its own neighbour: Slab.refresh packs on the handle's stream and copies the packed layers into
+    its own halos.  The caller may by then work on another stream than the one the slab was built on: the state q is
+    produced there (late: a sleep kernel runs first), so packing, local copies and sweeps must all be ordered behind it and
+    among themselves by events, not by luck.  Result: the single domain's, bit for bit."""
+    from paper_2503_07953_b200 import slab as S
+    case = make_case(3, 2, (33, 18, 23), W.BC_PERIODIC)
+    q = rough_state(case, 7)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    dt = 0.4 * g.cfl_dt(qd, 0.5)
+    for _ in range(2):
+        g.rk3_step(qd, dt)
+    g.check()
+    want = qd.cpu().numpy()
+    sl = S.Slab(case, rank=0, world=1)            # built on the default stream
+    assert sl.below == 0 and sl.above == 0
+    src = torch.from_numpy(q).cuda()
+    ql = torch.full_like(src, float("nan"))
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        torch.cuda._sleep(400_000_000)            # ~0.2 s during which q is still NaN
+        ql.copy_(src)
+        for _ in range(2):
+            sl.rk3_step(ql, dt)
+    # the caller's stream must see the result: Slab leaves the state on the handle's stream, so order the read behind it
+    sl.stream.synchronize()
+    side.synchronize()
+    sl.grid.check()
+    assert np.array_equal(ql.cpu().numpy(), want)
+    sl.close()
+    g.close()
 
 
 @pytest.mark.gpu
@@ -943,7 +1065,7 @@ def test_rhs_rough_state_viscous(torch, mfc, ndim, nfluids, n, bc):
     if min(n[:ndim]) > 1:
         assert np.abs(ref - inviscid)[mom].max() > 1e-2 * np.abs(ref[mom]).max()      # the terms are there
     got = gpu_rhs(torch, mfc, case, q)
-    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None)
+    worst, per = rel_err(got, ref, nfluids, ndim, noise if nfluids == 1 else None, t2_rows(nfluids, ndim))
     assert worst <= RHS_TOL, per
 
 
