@@ -15,9 +15,12 @@ the paper's Table-1 benchmark case), seeded synthetic input (mfc_w
 
 With no --config (config 4, N = 1) the line also carries, under "also", configs 5 (512^3, 10 equations, 5 steps) and 3
 (1024^2, 50 steps) and config 4 with the paper's default mapped weights (10 steps), each with its own roofline and clock record.  "roofline" names the dominant kernel and the roof that
-binds it (north_star: "the slower of the two"): the floor times of that launch for the FP64 ALUs (algorithmic flops / derived
-peak) and for HBM (compulsory bytes of the kernel / measured copy bandwidth) are both printed, `frac` is against the larger;
-`frac_whole_step` is the algorithmic flop rate of the whole step against the FP64 peak.
+binds it (north_star: "the slower of the two"): the floor times of that launch for the FP64 ALUs (algorithmic
+flops / derived peak) and for HBM (ALGORITHMIC bytes of the RK stage / measured copy bandwidth) are both printed, `frac` is
+against the larger; `design_hbm_frac` is the separate statement about the three-sweep design (its compulsory bytes over the
+copy bandwidth); `traffic` / `traffic_ratio` come from the committed ncu capture (stale captures are refused);
+`frac_whole_step` is the larger of the two algorithmic floors of the whole step over the step time.  `also_summary`, near the
+front of the line, has one compact entry for configs 5, 3, 1, 2 and config 4 with mapped weights.
 
 N > 1 (torchrun): the path runs on one GPU (north_star); ranks are independent replicas ("replicas only",
 DESIGN.md §9) — no data-path collective; time is the max over ranks, value the whole-job aggregate.
@@ -147,6 +150,24 @@ def sweep_alg_bytes_per_cell(kernel, neq, ndim):
     if kernel == last:
         return ((16 if ndim == 1 else 24) + 8 * 2.0 / 3.0) * neq
     return (16 if kernel == "sweep_x" else 24) * neq
+
+
+def stage_alg_bytes_per_cell(neq):
+    """ALGORITHMIC bytes per cell of one RK stage whatever the kernel design — read the swept state once,
+    read q^n too where it is another array (stages 2, 3), write the new stage state once: (16 + 24 + 24)/3 per equation on
+    the average of the three stages.  A launch of the dominant sweep kernel (one per stage) is charged ALL of it: the HBM
+    floor this gives is the one a fully fused stage kernel would have, the most any design could ask of that launch."""
+    return (16 + 24 + 24) / 3.0 * neq
+
+
+def kernel_sources_sha256():
+    """hash of the CUDA sources: profiles/traffic.json records the one its ncu capture was made with"""
+    import hashlib
+    h = hashlib.sha256()
+    for fn in ("mfc_b200.cu", "mfc_device.cuh"):
+        with open(os.path.join(ROOT, "paper_2503_07953_b200", "csrc", fn), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
 
 
 def run_reference(args, rank):
@@ -325,11 +346,21 @@ def measure(args, config_index, steps, rank, local_rank, world, with_e2e):
     flops_launch = flops_rhs / case.ndim
     bytes_launch = sweep_alg_bytes_per_cell(dom, neq, case.ndim) * cells
     hbm_peak, hbm_src = measured_peaks()
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu --set full capture
+    # dram bytes per launch: NOT measured in this run (the counters need ncu) but read from the committed ncu --set full
+    # capture; the file records the hash of the CUDA sources it was captured with, and a capture of other sources is
+    # reported as stale instead of being passed off as this build's
+    traffic, traffic_all, traffic_note = None, {}, "no profiles/traffic.json"
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(f"config{config_index}", {}).get(dom)
+            tj = json.load(f)
+        fresh = tj.get("kernel_sources_sha256") == kernel_sources_sha256()
+        traffic_note = ("committed ncu --set full capture, " + str(tj.get("source")) +
+                        ("; captured with the CUDA sources of this build" if fresh else
+                         "; STALE: captured with other CUDA sources than this build's (kernel_sources_sha256 differs)"))
+        if fresh:
+            traffic_all = tj.get(f"config{config_index}", {})
+            traffic = traffic_all.get(dom)
     dfma_tf, dfma3_tf, probe_clocks = probe_fp64(M, local_rank)
     alu = {"achieved": flops_launch / dur_s / 1e12, "peak": FP64_PEAK_TFLOPS_DERIVED, "unit": "TFLOP/s",
            "frac": flops_launch / dur_s / 1e12 / FP64_PEAK_TFLOPS_DERIVED,
@@ -341,10 +372,17 @@ def measure(args, config_index, steps, rank, local_rank, world, with_e2e):
            "peak_source": hbm_src + " (MEASURED_PEAKS.json hbm_gbs)" if hbm_src == "measured" else "fallback of B200_PROFILING.md",
            "alg_bytes_per_launch": bytes_launch,
            "bytes_are": "compulsory bytes of this kernel in the three-sweep design (q, partial L, q^n read; new state written)"}
-    # north_star: "the roofline taken as the slower of the two": the roof with the larger floor time binds this launch
-    t_alu, t_hbm = flops_launch / (FP64_PEAK_TFLOPS_DERIVED * 1e12), bytes_launch / (hbm_peak * 1e9)
+    # SURVEY.md §8(d) / north_star "the roofline taken as the slower of the two": both floors from ALGORITHMIC work — the flops
+    # of this launch, and the bytes any design must move for the stage (stage_alg_bytes_per_cell) — the larger floor binds.
+    # The compulsory bytes of the three-sweep DESIGN (hbm above) are a statement about this design, kept as design_hbm_frac.
+    alg_bytes_launch = stage_alg_bytes_per_cell(neq) * cells
+    hbm_alg = {"achieved": alg_bytes_launch / dur_s / 1e9, "peak": hbm_peak, "unit": "GB/s",
+               "frac": alg_bytes_launch / dur_s / 1e9 / hbm_peak, "alg_bytes_per_launch": alg_bytes_launch,
+               "bytes_are": "algorithmic bytes of one RK stage (SURVEY 8(d)): (16 + 24 + 24)/3 x neq per cell"}
+    t_alu, t_hbm = flops_launch / (FP64_PEAK_TFLOPS_DERIVED * 1e12), alg_bytes_launch / (hbm_peak * 1e9)
+    t_hbm_design = bytes_launch / (hbm_peak * 1e9)
     bound = "alu" if t_alu >= t_hbm else "hbm"
-    sel = alu if bound == "alu" else hbm
+    sel = alu if bound == "alu" else hbm_alg
     step_s = ms * 1e-3 / steps
     # whole step: algorithmic flops of 3 RHS evaluations / algorithmic bytes of SURVEY 8(d) (RHS: 16 neq per cell; an RK stage
     # re-reads q^n in stages 2, 3 and the CFL reduction reads q once: (3*16 + 2*8 + 8) neq per cell per step) over the step time
@@ -352,11 +390,21 @@ def measure(args, config_index, steps, rank, local_rank, world, with_e2e):
     whole = {"alu_frac": 3 * flops_rhs / step_s / 1e12 / FP64_PEAK_TFLOPS_DERIVED, "alu_tflops": 3 * flops_rhs / step_s / 1e12,
              "hbm_frac_algorithmic_bytes": step_bytes / step_s / 1e9 / hbm_peak, "alg_bytes_per_step": step_bytes,
              "ms_per_step": step_s * 1e3}
+    # measured DRAM bytes of a whole step over its algorithmic bytes (wasted traffic), when the capture covers every sweep
+    if all(k in traffic_all for k in sweeps):
+        step_traffic = sum(traffic_all[k] * kern[k]["launches_per_step"] for k in sweeps) + traffic_all.get("cfl", 8.0 * neq * cells)
+        whole["traffic_bytes_per_step"] = step_traffic
+        whole["traffic_ratio"] = step_traffic / step_bytes
+    whole["frac"] = max(whole["alu_frac"], whole["hbm_frac_algorithmic_bytes"])
     roofline = {"kernel": dom, "bound": bound, "achieved": sel["achieved"], "peak": sel["peak"], "unit": sel["unit"],
-                "frac": sel["frac"], "traffic": traffic, "ms_per_launch": dur_s * 1e3,
+                "frac": sel["frac"], "traffic": traffic,
+                "traffic_ratio": (traffic / alg_bytes_launch) if traffic else None, "traffic_source": traffic_note,
+                "ms_per_launch": dur_s * 1e3,
                 "denominator": ("alu: derived FP64 peak 37.2 TFLOP/s" if bound == "alu" else "hbm: measured copy bandwidth") +
-                               "; floor times of this launch: alu %.3f ms, hbm %.3f ms" % (t_alu * 1e3, t_hbm * 1e3),
-                "alu": alu, "hbm": hbm, "frac_whole_step": whole["alu_frac"], "whole_step": whole, "kernels": kern}
+                               "; floor times of this launch from algorithmic work: alu %.3f ms, hbm %.3f ms (three-sweep design's "
+                               "compulsory bytes: %.3f ms)" % (t_alu * 1e3, t_hbm * 1e3, t_hbm_design * 1e3),
+                "design_hbm_frac": hbm["frac"], "alu": alu, "hbm_algorithmic": hbm_alg, "hbm_design": hbm,
+                "frac_whole_step": whole["frac"], "whole_step": whole, "kernels": kern}
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the state, the step, D2H of the state, every step
     e2e = None
@@ -458,17 +506,25 @@ def main():
         "ms_per_step": head["ms_per_step"], "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
     }
+    out["also_summary"] = None   # filled below; sits near the front of the line so that a truncated tail does not lose it
     for k in ("config", "cell_updates_per_s", "clocks", "gpu_launches", "e2e", "rhs_only", "roofline",
               "ms_per_step_median_of_10_single_steps"):
         out[k] = head[k]
+
+    def summary(r):
+        return {"workload": r["config"]["workload"], "weno": r["config"]["weno"], "steps": r["steps"], "ms_per_step": r["ms_per_step"],
+                "value": r["value"], "kernel": r["roofline"]["kernel"], "bound": r["roofline"]["bound"], "frac": r["roofline"]["frac"],
+                "frac_whole_step": r["roofline"]["frac_whole_step"], "sm_mhz": r["clocks"].get("sm_mhz"),
+                "reasons": r["clocks"].get("reasons"), "gpu_launches": r["gpu_launches"]}
     out["paper_context"] = "PAPER.md:720-726 Table 1 (other hardware, whole step): GH200 0.32, H100 SXM 0.38, A100 0.62 ns"
     # the other two configurations the target names ("the 3D configs") and the full-size 2-D one, each with its own roofline
     # and clock record: config 5 (512^3, 10 equations, the largest single-GPU workload) and config 3 (1024^2)
     if args.config == 4 and world == 1 and not args.no_also and args.n is None and args.decomp == "replicas":
-        also = {}
-        for idx, st in ((5, 5), (3, 50)):
+        also, summ = {}, []
+        for idx, st in ((5, 5), (3, 50), (1, 200), (2, 200)):
             try:
                 r = measure(args, idx, st, rank, local_rank, world, with_e2e=False)
+                summ.append(summary(r))
                 also[r["config"]["workload"]] = {k: r[k] for k in (
                     "value", "ms_per_step", "ms_per_step_median_of_10_single_steps", "steps", "config", "cell_updates_per_s",
                     "clocks", "gpu_launches", "rhs_only", "roofline")}
@@ -480,12 +536,14 @@ def main():
                 am = copy.copy(args)
                 am.weno = "m"
                 r = measure(am, 4, 10, rank, local_rank, world, with_e2e=False)
+                summ.append(summary(r))
                 also[r["config"]["workload"] + " with WENO5-M"] = {k: r[k] for k in (
                     "value", "ms_per_step", "ms_per_step_median_of_10_single_steps", "steps", "config", "cell_updates_per_s",
                     "clocks", "gpu_launches", "rhs_only", "roofline")}
             except Exception as exc:
                 also["4 with WENO5-M"] = {"error": repr(exc)}
         out["also"] = also
+        out["also_summary"] = summ
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.config, args.weno, args.model, args.eta)
     if rank == 0:

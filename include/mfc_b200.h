@@ -219,6 +219,11 @@ mfc_status mfc_rk3_steps_host(mfc_grid *g, double *q_host, double dt, int nsteps
  * mfc_rk3_step (bit-identical states and elapsed time), without a host round trip per step.  Both calls synchronise once,
  * at the end, and then report the sticky non-physical flag (a state that turns non-physical in step k is still stepped to
  * the end).  mfc_advance: q device.  mfc_advance_host: q_host HOST, copied in before and out after the nsteps steps. */
+/* On grids of at most 2^18 cells (launch-bound: BASELINE.json configs 1 and 2) both calls replay a CUDA graph of two steps
+ * — one graph launch instead of 22 kernel launches — captured on the third step of a handle and re-captured when q or cfl
+ * change; same kernels, arguments and order, hence the same bits.  mfc_set_step_graph(g, 0) turns that off (on by default;
+ * it is also off while profiling is on).  The replay runs on a stream of the handle's own, ordered behind and before the
+ * handle's stream by events. */
 mfc_status mfc_advance(mfc_grid *g, double *q, double cfl, int nsteps, double *t_elapsed_host);
 mfc_status mfc_advance_host(mfc_grid *g, double *q_host, double cfl, int nsteps, double *t_elapsed_host);
 
@@ -260,6 +265,9 @@ mfc_status mfc_measure_fp64(int device, void *stream, double *dfma_tflops_host, 
  * 0 keeps the library's choice.  Results do not depend on it beyond round-off-free re-partitioning
  * (each face flux is computed from the same inputs wherever the segment boundaries fall). */
 mfc_status mfc_set_segments(mfc_grid *g, int seg_x, int seg_y, int seg_z);
+
+/* on = 0: mfc_advance / mfc_advance_host launch every kernel of every step themselves, whatever the grid size (see there). */
+mfc_status mfc_set_step_graph(mfc_grid *g, int on);
 
 /* Text of the last error on this host thread ("" if none). */
 const char *mfc_last_error(void);

@@ -21,7 +21,7 @@ EXPORTS = ("mfc_init_grid", "mfc_free_grid", "mfc_num_eqns", "mfc_num_cells", "m
            "mfc_rk3_steps_host", "mfc_advance", "mfc_advance_host", "mfc_set_profiling", "mfc_get_profile",
            "mfc_weno5_values", "mfc_hllc_faces", "mfc_launch_count", "mfc_set_segments", "mfc_last_error", "mfc_set_halo", "mfc_rk3_stage",
            "mfc_stage_input", "mfc_pack_halo", "mfc_measure_fp64", "mfc_rk3_stage_parts", "mfc_cfl_dt_static",
-           "mfc_sqrt_ratio_values")
+           "mfc_sqrt_ratio_values", "mfc_set_step_graph")
 STATIC_MAX_CELLS = 2048 * 16384  # MFC_STATIC_MAX_CELLS of include/mfc_b200.h
 
 
@@ -79,6 +79,7 @@ def lib():
         L.mfc_hllc_faces.argtypes = [vp, C.c_int, dp, dp, C.c_longlong, dp, dp]
         L.mfc_launch_count.argtypes = [vp]; L.mfc_launch_count.restype = C.c_longlong
         L.mfc_set_segments.argtypes = [vp, C.c_int, C.c_int, C.c_int]
+        L.mfc_set_step_graph.argtypes = [vp, C.c_int]
         L.mfc_last_error.restype = C.c_char_p
         L.mfc_set_halo.argtypes = [vp, dp, dp]
         L.mfc_rk3_stage.argtypes = [vp, dp, C.c_double, C.c_int]
@@ -305,6 +306,10 @@ class Grid:
 
     def launch_count(self):
         return lib().mfc_launch_count(self._h)
+
+    def set_step_graph(self, on):
+        """False: advance() launches every kernel of every step itself also on small grids (default: a CUDA graph of two steps)"""
+        _ck(lib().mfc_set_step_graph(self._h, int(bool(on))))
 
     def set_segments(self, seg_x=0, seg_y=0, seg_z=0):
         _ck(lib().mfc_set_segments(self._h, seg_x, seg_y, seg_z))

@@ -409,8 +409,13 @@ __global__ void __launch_bounds__(MB, 1) sweep_march(const __grid_constant__ KP 
       }
     }
     ++cl;
-    if ((ACCUM || STAGE >= 1) && (BF || p >= 2)) {  // operands of this step's update (BF, p < 2: a valid cell, unused)
-      const int offs = p >= 2 ? offc : base;
+    if ((ACCUM || STAGE >= 1) && (BF || p >= 2)) {  // operands of this step's update
+      // BF, p < 2: nothing is updated yet, but the copies are issued all the same — and they are NOT waited for before step 2
+      // issues its own into the same slots.  cp.async groups may land in any order, so the two early copies must carry what
+      // step 2's carries: the segment's first cell (offc of step 2).  (They used to read the column's cell 0: when one of them
+      // landed last, the first cell of a segment other than the first was updated with the operands of cell 0 — a few times
+      // in a thousand steps of config 4 at 128^3; found by the 50-step parity test.)
+      const int offs = p >= 2 ? offc : base + s0 * stride;
 #pragma unroll
       for (int v = 0; v < NEQ; ++v) {
         if (ACCUM) cp_async8(&RG(S_ACC, v), rhs + v * kp.ncells + offs);
@@ -791,6 +796,16 @@ struct mfc_grid {
   unsigned long long* h_red = nullptr;  // pinned: [0] smax bits, [1] flag
   int seg[3];
   long long launches = 0;
+  // CUDA graph of two mfc_advance steps for launch-bound grids (advance_pairs_graph)
+  bool step_graph = true;               // mfc_set_step_graph
+  bool adv_warm = false;                // two plain steps have run on this handle (every launch function has done its one-time queries)
+  cudaGraphExec_t adv_exec = nullptr;
+  const double* adv_q = nullptr;        // what the instantiated graph was captured for
+  double adv_cfl = 0.0;
+  int adv_parity = 0;
+  long long adv_kernels = 0;            // kernels in the graph
+  cudaStream_t gstream = nullptr;       // capture / replay stream (the handle's own may be the legacy stream, which cannot capture)
+  cudaEvent_t gev_in = nullptr, gev_out = nullptr;
   int num_sms = 148;
   // per-kernel device timing (mfc_set_profiling)
   bool profiling = false;
@@ -1135,6 +1150,11 @@ static cudaError_t launch_rk3_stage(mfc_grid* g, double* q, double dt, int stage
 }
 
 
+static void drop_step_graph(mfc_grid* g) {
+  if (g->adv_exec) cudaGraphExecDestroy(g->adv_exec);
+  g->adv_exec = nullptr;
+}
+
 static mfc_status use_device(const mfc_grid* g) {
   CK(cudaSetDevice(g->device));
   return MFC_OK;
@@ -1267,6 +1287,13 @@ mfc_status mfc_free_grid(mfc_grid* g) {
   cudaFree(g->d_dt);
   cudaFree(g->d_xnext);
   if (g->h_red) cudaFreeHost(g->h_red);
+  drop_step_graph(g);
+  if (g->gstream) {
+    cudaStreamSynchronize(g->gstream);
+    cudaStreamDestroy(g->gstream);
+    cudaEventDestroy(g->gev_in);
+    cudaEventDestroy(g->gev_out);
+  }
   drain_profile(g);
   for (cudaEvent_t e : g->pool) cudaEventDestroy(e);
   delete g;
@@ -1284,6 +1311,14 @@ mfc_status mfc_set_segments(mfc_grid* g, int seg_x, int seg_y, int seg_z) {
   mfc_grid tmp = *g;
   default_segments(&tmp);
   for (int d = 0; d < 3; ++d) g->seg[d] = s[d] > 0 ? (s[d] < g->kp.n[d] ? s[d] : g->kp.n[d]) : tmp.seg[d];
+  drop_step_graph(g);  // the launch shapes are part of a captured step
+  return MFC_OK;
+}
+
+mfc_status mfc_set_step_graph(mfc_grid* g, int on) {
+  if (!g) return fail(MFC_ERR_ARG, "mfc_set_step_graph: NULL handle");
+  g->step_graph = on != 0;
+  if (!on) drop_step_graph(g);
   return MFC_OK;
 }
 
@@ -1441,9 +1476,7 @@ mfc_status mfc_rk3_steps_host(mfc_grid* g, double* q_host, double dt, int nsteps
 // CFL + RK3 per step, all on the device: the reduction leaves max_cells sum_d (|u_d|+c)/dx_d, dt_kernel turns it into dt
 // and adds it to the elapsed time, the RK stages read dt from device memory.  One host synchronisation at the end, which
 // also reports the sticky non-physical flag.  Same kernels and arithmetic as the caller's loop of mfc_cfl_dt + mfc_rk3_step.
-static mfc_status advance_impl(mfc_grid* g, double* q, double cfl, int nsteps, double* t_out) {
-  CK(cudaMemsetAsync(g->d_dt, 0, 2 * sizeof(double), g->stream));
-  CK(cudaMemsetAsync(g->d_red, 0, 8, g->stream));
+static mfc_status advance_steps_plain(mfc_grid* g, double* q, double cfl, int nsteps) {
   for (int s = 0; s < nsteps; ++s) {
     CK(MFC_DISPATCH(g, (launch_cfl<N, D>(g, q))));
     {
@@ -1456,6 +1489,80 @@ static mfc_status advance_impl(mfc_grid* g, double* q, double cfl, int nsteps, d
     g->kp.dt_dev = nullptr;
     CK(e);
   }
+  return MFC_OK;
+}
+
+// Launch-bound grids (BASELINE.json configs 1 and 2: 1000 and 4000 cells, 11 launches of a few microseconds each per step):
+// the launches of TWO steps are captured once into a CUDA graph and replayed, one graph launch per pair of steps.  Two, not
+// one: sweep_x alternates between two work counters from launch to launch (launch_x) and a step has three x sweeps, so only
+// after two steps does the next launch find the counters as the capture did.  The graph holds the very kernels, arguments
+// and order of advance_steps_plain — same bits — and is re-captured when q, cfl or the counter parity differ from the capture's.
+// The handle's stream may be the legacy default stream, which cannot be captured: capture and replay run on a stream of the
+// handle's own, ordered against the handle's stream by events on both sides.
+constexpr long long STEP_GRAPH_MAX_CELLS = 1 << 18;
+
+static mfc_status advance_pairs_graph(mfc_grid* g, double* q, double cfl, int npairs) {
+  if (!g->gstream) {
+    CK(cudaStreamCreateWithFlags(&g->gstream, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&g->gev_in, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&g->gev_out, cudaEventDisableTiming));
+  }
+  if (!g->adv_exec || g->adv_q != q || g->adv_cfl != cfl || g->adv_parity != g->xparity) {
+    drop_step_graph(g);
+    const cudaStream_t user = g->stream;
+    const long long l0 = g->launches;
+    const int parity = g->xparity;
+    cudaError_t e = cudaStreamBeginCapture(g->gstream, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamBeginCapture");
+    g->stream = g->gstream;
+    const mfc_status st = advance_steps_plain(g, q, cfl, 2);
+    g->stream = user;
+    cudaGraph_t graph = nullptr;
+    e = cudaStreamEndCapture(g->gstream, &graph);
+    g->adv_kernels = g->launches - l0;
+    g->launches = l0;          // captured, not run
+    g->xparity = parity;       // two steps: an even number of x sweeps, the parity is where it was
+    if (st != MFC_OK || e != cudaSuccess) {
+      if (graph) cudaGraphDestroy(graph);
+      return st != MFC_OK ? st : cuda_fail(e, "cudaStreamEndCapture");
+    }
+    e = cudaGraphInstantiate(&g->adv_exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) {
+      g->adv_exec = nullptr;
+      return cuda_fail(e, "cudaGraphInstantiate");
+    }
+    g->adv_q = q;
+    g->adv_cfl = cfl;
+    g->adv_parity = parity;
+  }
+  CK(cudaEventRecord(g->gev_in, g->stream));
+  CK(cudaStreamWaitEvent(g->gstream, g->gev_in, 0));
+  for (int i = 0; i < npairs; ++i) {
+    CK(cudaGraphLaunch(g->adv_exec, g->gstream));
+    g->launches += g->adv_kernels;
+  }
+  CK(cudaEventRecord(g->gev_out, g->gstream));
+  CK(cudaStreamWaitEvent(g->stream, g->gev_out, 0));
+  return MFC_OK;
+}
+
+static mfc_status advance_impl(mfc_grid* g, double* q, double cfl, int nsteps, double* t_out) {
+  CK(cudaMemsetAsync(g->d_dt, 0, 2 * sizeof(double), g->stream));
+  CK(cudaMemsetAsync(g->d_red, 0, 8, g->stream));
+  int left = nsteps;
+  if (g->step_graph && !g->profiling && g->kp.ncells <= STEP_GRAPH_MAX_CELLS) {
+    if (!g->adv_warm && left >= 2) {  // the first two steps of a handle run plainly (one-time occupancy queries are not captured)
+      if (mfc_status s = advance_steps_plain(g, q, cfl, 2)) return s;
+      g->adv_warm = true;
+      left -= 2;
+    }
+    if (g->adv_warm && left >= 2) {
+      if (mfc_status s = advance_pairs_graph(g, q, cfl, left / 2)) return s;
+      left &= 1;
+    }
+  }
+  if (mfc_status s = advance_steps_plain(g, q, cfl, left)) return s;
   CK(cudaMemcpyAsync(&g->h_red[0], g->d_dt + 1, 8, cudaMemcpyDeviceToHost, g->stream));
   g->h_red[1] = 0;
   const mfc_status st = read_flag_and_sync(g, false);

@@ -280,7 +280,7 @@ def test_rhs_full_size_config5_sampled(torch, mfc):
 # ------------------------------------------------------------------ full-size parity THROUGH THE FUSED-STAGE KERNELS
 # mfc_advance (what bench.py times) = CFL reduction + the STAGE = 1, 2, 3 instantiations of the sweeps, at the launch shape
 # of the full-size grids (64-cell y/z segments, one-wave x grid with the dynamic chunk counter).  PAPER.md:207-211 with 137-143.
-def _advance_vs_oracle(torch, mfc, case, nsteps=1):
+def _advance_vs_oracle(torch, mfc, case, nsteps=1, exact_time=True):
     q = W.initial_state(case)
     orc = O.Oracle(case)
     ref = q.copy()
@@ -295,7 +295,10 @@ def _advance_vs_oracle(torch, mfc, case, nsteps=1):
         t_ref += dt
     got = qd.cpu().numpy()
     g.close()
-    assert t_gpu == t_ref  # the device-side time step is the oracle's, bit for bit
+    if exact_time:
+        assert t_gpu == t_ref  # the device-side time step is the oracle's, bit for bit
+    else:                      # many steps: the states differ in their last digits, and so do the time steps taken from them
+        assert abs(t_gpu - t_ref) <= 1e-12 * t_ref
     # the bar of a state after RK3 steps; the increment q^{n+1} - q^n is held to the one-RHS bar relative to its own size
     worst, per = rel_err(got, ref, case.nfluids, case.ndim)
     inc_worst, inc_per = rel_err(got - q, ref - q, case.nfluids, case.ndim)
@@ -473,6 +476,111 @@ def test_rk3_steps_configs(torch, mfc, index, n, nsteps):
     got = qd.cpu().numpy()
     worst, per = rel_err(got, ref, case.nfluids, case.ndim)
     assert worst <= STEP_TOL, per
+
+
+# north_star: "1e-9 after 100 RK3 steps ... on all 5 configs" — at, or near, the sizes bench.py times (configs 1 and 2 run at
+# full size above).  The reference's time step is given to both sides (A9); ~2 min of reference time on 16 host cores.
+@pytest.mark.parametrize("index,n,nsteps", [(3, None, 100), (4, 128, 50), (5, 96, 20)])
+def test_rk3_steps_near_full_size(torch, mfc, capsys, index, n, nsteps):
+    case = W.config(index, n=n)   # config 3: 1024^2 in full
+    q = W.initial_state(case)
+    orc = O.Oracle(case)
+    g = mfc.Grid.from_case(case)
+    qd = torch.from_numpy(q).cuda()
+    ref = q.copy()
+    for s in range(nsteps):
+        dt_ref = orc.cfl_dt(ref, case.cfl)
+        orc.rk3_step(ref, dt_ref)
+        assert orc.bad == 0
+        g.rk3_step(qd, dt_ref)
+    g.check()
+    got = qd.cpu().numpy()
+    worst, per = rel_err(got, ref, case.nfluids, case.ndim)
+    g.close()
+    with capsys.disabled():
+        print(f"\n[{nsteps} steps, {case.name} {case.n}] worst e_v = {worst:.2e} {per}")
+        if worst > STEP_TOL:   # where: a failure here is a handful of cells or a whole block of work, and the message should say which
+            for v in range(case.neq):
+                off = np.argwhere(np.abs(got[v] - ref[v]) > 1e-7 * np.abs(ref[v]).max())
+                if len(off):
+                    print(f"  variable {v}: {len(off)} cells off, (k, j, i) from {off.min(0)} to {off.max(0)}, NaN: {int(np.isnan(got[v]).sum())}")
+    assert worst <= STEP_TOL, per
+
+
+def test_advance_full_size_config4_ten_steps(torch, mfc, capsys):
+    """256^3, the grid bench.py times, ten adaptive steps through mfc_advance (device-side dt, fused-stage kernels) against ten
+    reference steps with the reference's own dt: state within the 100-step bar, elapsed time to rounding."""
+    worst, per, inc_worst, inc_per = _advance_vs_oracle(torch, mfc, W.config(4), nsteps=10, exact_time=False)
+    with capsys.disabled():
+        print(f"\n[10 steps of mfc_advance, config 4 at 256^3] worst e_v = {worst:.2e} {per}; increments {inc_per}")
+    assert worst <= STEP_TOL, per
+    assert inc_worst <= 1e-7, inc_per
+
+
+def test_fused_stage_sweeps_are_deterministic_run_to_run(torch, mfc):
+    """The same step on the same state gives the same bits, every time.  Found with the 50-step parity case above (one run in
+    five failed): the branch-free z sweep issued its operand copies (cp.async) in steps 0 and 1 of a segment without waiting
+    for them, step 2 issued the real ones into the same shared-memory slots, and cp.async groups may land in any order —
+    about once in a thousand steps of this grid (32-cell z segments) the first cell of a segment was updated with the
+    operands of the column's cell 0.  1500 repetitions of one step and of one RHS evaluation, bit-compared."""
+    case = W.config(4, n=128)
+    q0 = torch.from_numpy(W.initial_state(case)).cuda()
+    g = mfc.Grid.from_case(case)
+    dt = 0.9 * g.cfl_dt(q0, case.cfl)
+    ref, rref, r = None, None, torch.empty_like(q0)
+    differing = [0, 0]
+    for rep in range(1500):
+        qd = q0.clone()
+        g.rk3_step(qd, dt)
+        g.rhs(q0, r)
+        if ref is None:
+            ref, rref = qd.clone(), r.clone()
+        else:
+            differing[0] += int(not torch.equal(qd, ref))
+            differing[1] += int(not torch.equal(r, rref))
+    g.check()
+    g.close()
+    assert differing == [0, 0], differing
+
+
+# ------------------------------------------------------------------ launch-bound grids: mfc_advance replays a CUDA graph
+@pytest.mark.parametrize("index,n", [(1, None), (2, None), (3, 96), (4, 24)])
+def test_advance_step_graph_is_bit_identical_to_plain_launches(torch, mfc, capsys, index, n):
+    """On grids of at most 2^18 cells mfc_advance replays a captured graph of two steps (one launch per pair of steps instead
+    of 22).  Same kernels, arguments and order: states, elapsed time and launch count equal those of the plain path bit for
+    bit — for odd and even step counts, after a call that flips the x sweep's counter parity in between, on another state
+    array, with another cfl, and through the host-buffer entry point."""
+    import time
+    case = W.config(index, n=n)
+    q = W.initial_state(case)
+    res = {}
+    for graphs in (False, True):
+        g = mfc.Grid.from_case(case)
+        g.set_step_graph(graphs)
+        qd = torch.from_numpy(q).cuda()
+        qe = torch.from_numpy(q).cuda()
+        ts = [g.advance(qd, case.cfl, 7)]             # 2 plain + 2 pairs + 1 plain
+        ts.append(g.advance(qd, case.cfl, 6))         # 3 pairs
+        g.rk3_step(qd, 0.5 * g.cfl_dt(qd, case.cfl))  # three x sweeps: the counter parity flips -> re-capture
+        ts.append(g.advance(qd, case.cfl, 5))
+        ts.append(g.advance(qe, 0.7 * case.cfl, 4))   # another array, another cfl -> re-capture
+        ts.append(g.advance(qd, case.cfl, 1))
+        ts.append(g.advance(qd, case.cfl, 0))
+        h = qe.cpu().numpy().copy()
+        ts.append(g.advance_host(h, case.cfl, 6))
+        launches = g.launch_count()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        g.advance(qd, case.cfl, 400)
+        us = (time.perf_counter() - t0) * 1e6 / 400
+        res[graphs] = (qd.cpu().numpy(), qe.cpu().numpy(), h, ts, launches, us)
+        g.check()
+        g.close()
+    a, b = res[False], res[True]
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    assert a[3] == b[3] and a[4] == b[4]
+    with capsys.disabled():
+        print(f"\n[step graph, {case.name} {case.n}] {a[5]:.1f} us per step with plain launches, {b[5]:.1f} us with the two-step graph")
 
 
 def test_sod_to_final_time_adaptive_dt(torch, mfc):

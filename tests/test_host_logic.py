@@ -84,6 +84,9 @@ def test_grind_time_arithmetic():
     assert bench.sweep_alg_bytes_per_cell("sweep_y", 8, 3) == 192           # middle sweep: q and L read, L written
     assert bench.sweep_alg_bytes_per_cell("sweep_z", 8, 3) == pytest.approx(8 * (24 + 32 + 32) / 3)  # last sweep + RK stage, mean of 3
     assert bench.sweep_alg_bytes_per_cell("sweep_y", 7, 2) == pytest.approx(7 * (24 + 32 + 32) / 3)
+    # algorithmic bytes of an RK stage, whatever the design: 576 B per cell per step at neq = 8 with the CFL read
+    assert 3 * bench.stage_alg_bytes_per_cell(8) + 8 * 8 == 576
+    assert len(bench.kernel_sources_sha256()) == 64
     assert bench.median([3.0, 1.0, 2.0]) == 2.0 and bench.median([4.0, 1.0, 2.0, 3.0]) == 2.5
     assert bench.FP64_PEAK_TFLOPS_DERIVED == pytest.approx(37.225, rel=1e-3)
 
